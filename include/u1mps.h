@@ -1,0 +1,137 @@
+/* u1mps.h — C ABI of libu1mps.so: the charge-blocked two-site update of a U(1)-symmetric
+ * matrix-product state (arXiv:2303.11409; citations are PAPER.md line numbers), hand-written CUDA
+ * for sm_100a (B200).  One GPU, one stream, no CPU fallback: every step of the path runs in
+ * kernels of this library; if no CUDA device is present every call returns U1MPS_ECUDA.
+ *
+ * State (Eq.15): {Gamma^[k], lambda^[k], c^[k]}.  0-based indexing: sites
+ * s = 0..M-1, bonds k = 0..M; site s has left bond s and right bond s+1.  c^[k] = number of
+ * particles on sites k..M-1 (reading S2), so bond 0 = {N}, bond M = {0}.  A bond is a list of charge
+ * sectors (c, n_k(c)), ascending c; inside a sector lambda is descending (reading S10).
+ * Gamma^[s] is a set of dense blocks Gamma^[s][c_l, c_r], n_s(c_l) x n_{s+1}(c_r), row-major
+ * complex128 (interleaved re,im), present only for occupation c_l - c_r in [0, d-1].
+ *
+ * Update (Eq.16; Eq.12; Eq.13/14 L94-104): steps a1 sector enumeration,
+ * a2 Theta(c) contraction, a3 one SVD per centre charge c, a4 global top-chi, a5 renormalise and
+ * scatter; a6 readouts.  See DESIGN.md for the data layout and each kernel.
+ *
+ * Conventions.  All functions return int: 0 = OK, negative = error (never throw, never abort).
+ * "host" / "device" says where a pointer must live.  The caller owns every pointer it passes;
+ * the library copies what it needs before returning (host U) or in stream order (device U: the
+ * buffer must stay valid until the stream has passed the call).  The arena and the stream given
+ * to u1mps_create are borrowed for the lifetime of the handle.  Calls marked [sync] synchronise
+ * the stream; all others only enqueue work (sector sizes stay on the device).
+ */
+#ifndef U1MPS_H
+#define U1MPS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct u1mps u1mps_t; /* opaque; created by u1mps_create, freed by u1mps_destroy */
+
+enum {
+  U1MPS_OK = 0,
+  U1MPS_EINVAL = -1,  /* bad index / size / occupation / null pointer */
+  U1MPS_ENOTU1 = -2,  /* host gate has an entry > 1e-14 that violates charge conservation (Eq.1) */
+  U1MPS_ESTAGED = -3, /* call not allowed in the current staging state (see u1mps_apply_two_site_gate) */
+  U1MPS_ENOMEM = -4,  /* arena too small for this call */
+  U1MPS_ECUDA = -5,   /* CUDA error (sticky), or no CUDA device */
+  U1MPS_ENOCONV = -6  /* Jacobi SVD hit the sweep limit on some sector (reported by [sync] calls) */
+};
+
+const char* u1mps_strerror(int code);
+
+/* Library build info: "u1mps <version> sm_100a". */
+const char* u1mps_version(void);
+
+/* Minimum arena size in bytes for a chain of M sites, local dimension d (occupations 0..d-1),
+ * N particles, bond dimension chi (<= 4096... see U1MPS_CHI_MAX): state + plan + the workspace of ONE worst-case gate.
+ * A larger arena lets u1mps_apply_gate_column process more gates of a column per launch. Returns 0 on bad arguments. */
+size_t u1mps_workspace_bytes(int M, int d, int N, int chi);
+#define U1MPS_CHI_MAX 4096
+#define U1MPS_D_MAX 8
+
+/* Create a handle on caller-allocated DEVICE memory (e.g. torch.empty(nbytes, dtype=uint8, device='cuda')).
+ * dev_arena must be 256-byte aligned; cuda_stream is a cudaStream_t (NULL = default stream).
+ * The state is undefined until u1mps_set_product_state or the import calls. */
+int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, size_t arena_bytes,
+                 void* cuda_stream);
+int u1mps_destroy(u1mps_t* h);
+
+/* |occ_0 ... occ_{M-1}>: occ is HOST int32[M], 0 <= occ < d, sum == N, else U1MPS_EINVAL.
+ * Every bond gets one sector of multiplicity 1, Gamma = [[1]], lambda = [1] (SURVEY §8(c) State). */
+int u1mps_set_product_state(u1mps_t* h, const int32_t* occ);
+
+/* Steps a1-a3 for sites (i, i+1), i in [0, M-2] (Eq.16; Eq.12 L91 per sector).
+ * U: complex128 interleaved, row-major d^2 x d^2, row = out_i*d + out_{i+1}, col = in_i*d + in_{i+1}
+ * (reading S3); host pointer if U_on_device == 0 (checked for charge conservation -> ENOTU1),
+ * device pointer otherwise (entries violating conservation are never read).  U need not be
+ * unitary (S13).  Leaves bond i+1 STAGED (V, sigma, W in the workspace); the only calls allowed
+ * while staged are u1mps_truncate(i), the u1mps_export_staged_* calls and u1mps_destroy. */
+int u1mps_apply_two_site_gate(u1mps_t* h, int i, const void* U, int U_on_device);
+
+/* Debug / test split of the call above: a1-a2 only (Theta staged), then a3. */
+int u1mps_stage_theta(u1mps_t* h, int i, const void* U, int U_on_device);
+int u1mps_stage_svd(u1mps_t* h);
+
+/* Steps a4-a5 on the staged gate ("largest chi singular values out of all ... and
+ * their corresponding bonds"; Eq.13/14): drop sigma <= cutoff (S7), order (sigma desc, c asc,
+ * j asc) (S8), keep the first chi (1 <= chi <= create-time chi; at least one), renormalise (S9),
+ * write lambda^[i+1], the sector table of bond i+1, Gamma^[i], Gamma^[i+1]. */
+int u1mps_truncate(u1mps_t* h, int i, int chi, double cutoff);
+
+int u1mps_apply_and_truncate(u1mps_t* h, int i, const void* U, int U_on_device, int chi, double cutoff);
+
+/* A whole column of mutually disjoint gates (the paper's gate-level parallelism, L179, folded
+ * onto one device): sites is HOST int32[n_gates], strictly increasing with gaps >= 2;
+ * U holds n_gates matrices back to back.  Same result as calling u1mps_apply_and_truncate for
+ * each gate in order.  All gates of the column share each kernel launch (split into several
+ * launches only if the arena is too small for the whole column). */
+int u1mps_apply_gate_column(u1mps_t* h, const int32_t* sites, int n_gates, const void* U,
+                            int U_on_device, int chi, double cutoff);
+
+/* a6 readouts.  out_host are HOST pointers.  All [sync]. */
+int u1mps_norm2(u1mps_t* h, double* out_host);                     /* exp(2 * accumulated log-norm) */
+int u1mps_log_norm(u1mps_t* h, double* out_host);                  /* sum over gates of 0.5 ln(sum sigma_kept^2) */
+int u1mps_expect_n(u1mps_t* h, int site, double* out_host);        /* canonical-form <n_site> */
+int u1mps_expect_n_all(u1mps_t* h, double* out_host /*[M]*/);      /* all sites, one launch */
+int u1mps_bond_entropy(u1mps_t* h, int bond, double* out_host);    /* -sum lambda^2 ln lambda^2 (natural log, S23) */
+int u1mps_bond_entropy_all(u1mps_t* h, double* out_host /*[M+1]*/);
+/* Sector table of a bond: writes up to cap (charge, count) pairs, ascending charge; *n_sectors = how many exist. */
+int u1mps_bond_info(u1mps_t* h, int bond, int32_t* n_sectors, int32_t* charges, int32_t* counts, int cap);
+int u1mps_bond_dims(u1mps_t* h, int32_t* dims_host /*[M+1]*/);
+/* Statistics since create / set_product_state: total discarded weight; of the LAST column or
+ * gate: kept bond dimension of its first gate, Jacobi sweeps used (max over sectors). */
+int u1mps_last_stats(u1mps_t* h, double* discarded_weight, int* kept, int* sweeps);
+
+/* Export / import (teacher-forced parity, checkpoints).  All [sync]; host buffers. */
+int u1mps_export_bond(u1mps_t* h, int bond, double* lambda_host, int cap);  /* ascending c, descending inside */
+/* Block Gamma^[site][cl, cr], row-major complex128, n_site(cl) x n_{site+1}(cr); cap in BYTES. */
+int u1mps_export_site(u1mps_t* h, int site, int cl, int cr, void* block_host, size_t cap);
+/* Replace the sector table and lambda of a bond.  charges ascending, counts >= 1, sum <= chi.
+ * Invalidates the blocks of sites bond-1 and bond: import them afterwards. */
+int u1mps_import_bond(u1mps_t* h, int bond, int n_sectors, const int32_t* charges, const int32_t* counts,
+                      const double* lambda_host);
+int u1mps_import_site(u1mps_t* h, int site, int cl, int cr, const void* block_host, size_t bytes);
+int u1mps_set_log_norm(u1mps_t* h, double log_norm, double discarded);
+
+/* Staged-gate read-back (valid between apply_two_site_gate / stage_* and truncate).  [sync]
+ * Candidate centre charges of the staged gate: for each, rows(c) and cols(c) of Theta(c). */
+int u1mps_staged_info(u1mps_t* h, int32_t* n_cand, int32_t* charges, int32_t* rows, int32_t* cols, int cap);
+/* After stage_theta: Theta(c), row-major rows x cols (row blocks ascending c_l, column blocks ascending c_r). */
+int u1mps_export_staged_theta(u1mps_t* h, int c, void* theta_host, size_t cap);
+/* After stage_svd / apply_two_site_gate: thin SVD of Theta(c): V rows x r, sigma r (descending), W r x cols,
+ * r = min(rows, cols), row-major.  Any of the three pointers may be NULL. */
+int u1mps_export_staged_svd(u1mps_t* h, int c, void* V_host, double* sigma_host, void* W_host);
+
+/* Number of kernels this handle has launched since create (for bench.py's gpu_launches). */
+int u1mps_launch_count(u1mps_t* h, long long* out_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* U1MPS_H */

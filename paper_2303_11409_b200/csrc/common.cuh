@@ -1,0 +1,83 @@
+// common.cuh — device-side data layout shared by the kernels of libu1mps.so (product path only;
+// nothing here is shared with oracle/).  See DESIGN.md §"Data layout in HBM".
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+typedef double2 cplx;  // complex128, interleaved (x = re, y = im), 16-byte aligned
+
+#define U1_TILE 32         // a2 / a5 tile edge
+#define U1_MAXSWEEP 40     // Jacobi sweep limit
+#define U1_PANEL 16        // max columns per Jacobi panel
+#define U1_ERR_WORKSPACE 1 // device error flag: plan does not fit the workspace
+#define U1_SVD_THREADS 512
+#define U1MPS_SORT_MAX 4096 // largest sector the in-smem bitonic sort takes (= U1MPS_CHI_MAX) // 16 warps: one per column pair of a panel-pair step
+
+// Persistent MPS state (all device pointers into the caller's arena).
+struct DevState {
+  int M, d, N, NC, chi;  // NC = N + 1 charge values 0..N
+  int* nb;               // [(M+1)*NC]  n_k(c): multiplicity of charge c on bond k (0 = absent)
+  int* ob;               // [(M+1)*NC]  exclusive scan of nb over c: offset of sector c in lambda^[k]
+  double* lam;           // [(M+1)*chi] lambda^[k], sectors ascending c, descending inside
+  cplx* gam;             // [M*gcap]    Gamma^[s] blocks, each row-major n_s(cl) x n_{s+1}(cr), tightly packed
+  long long gcap;        // chi*chi elements per site
+  long long* gamoff;     // [M*NC*d]    offset of block (cl, i = cl-cr) inside site s (scan over (cl,i))
+  double* scal;          // [0] log-norm, [1] discarded weight (total), [2] last w_kept, [3] last w_all
+  int* err;              // [0] sticky device error flag, [1] sweeps used (max), [2] non-converged blocks
+};
+
+// Per-launch plan for a batch ("chunk") of G disjoint gates.  Entry e = g*NC + c is the candidate
+// centre charge c of gate g (rows == 0 means "not a candidate").
+struct Plan {
+  int* site;         // [G] left site of gate g
+  cplx* U;           // [G*d^4] gate matrices
+  int* rows;         // [G*NC] rows(c) = sum_i n_L(c+i)
+  int* cols;         // [G*NC] cols(c) = sum_j n_R(c-j)
+  long long* goff;   // [G*NC+1] offset of the stacked (m+n) x n column-major Jacobi matrix of entry e
+  int* svoff;        // [G*NC+1] exclusive scan of n = min(rows, cols): offset in the sigma pool
+  int* t2pref;       // [G*NC*d*d+1] a2 tile prefix over (e, i, j)
+  int* t5pref;       // [G*NC*2+1] a5 tile prefix over (e, part)  part 0 = V, 1 = W
+  int* blk;          // [G*NC] compact list of entries with n > 0
+  int* pitem_e;      // [cap] Jacobi panel-pair items: entry e
+  int* pitem_k;      // [cap] ... pair slot k
+  int* iitem_e;      // [cap] intra-panel items: entry e
+  int* iitem_p;      // [cap] ... panel
+  int* tmpa;         // [G*NC+1] scratch: pair-item offset per entry
+  int* tmpb;         // [G*NC+1] scratch: intra-item offset per entry
+  int* cnt;          // [8] 0: #blk, 1: #pair items, 2: #intra items, 3: max panels, 4: a2 tiles, 5: a5 tiles, 7: a4 CTA counter
+  int* flags;        // [G*NC*U1_MAXSWEEP] per entry, per sweep: 1 if any rotation happened
+  int* keep;         // [G*NC] kept singular values per entry (a4)
+  int* perm;         // [pool] sorted position -> column index
+  double* sv;        // [pool] unsorted column norms
+  double* svs;       // [pool] sorted descending
+  double* gate_w;    // [2*G] per gate: kept weight, total weight (a4)
+  cplx* W;           // workspace for the stacked Jacobi matrices
+  long long wcap;    // capacity of W in elements
+  int poolcap;       // capacity of sv / svs / perm
+  int itemcap;       // capacity of the item lists
+};
+
+__host__ __device__ inline int u1_ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+// Panel width for a block with `mt` = m + n stacked rows and n columns; smem_elems = capacity of the
+// staging buffer in complex elements.  Returns b (columns per panel); *in_smem says whether two
+// panels fit in shared memory.
+__host__ __device__ inline int u1_panel_width(int mt, int n, long long smem_elems, int* in_smem) {
+  if ((long long)mt * 2 * U1_PANEL <= smem_elems) { *in_smem = 1; return U1_PANEL; }
+  if ((long long)mt * U1_PANEL <= smem_elems) { *in_smem = 1; return U1_PANEL / 2; }
+  *in_smem = 0;
+  return U1_PANEL;
+}
+
+// Host-side launchers (one per kernel file).  `stream` is the handle's stream.
+struct LaunchCfg { int sms; int svd_grid; int svd_smem; cudaStream_t stream; long long* launches; };
+
+void u1_launch_plan(const DevState& S, const Plan& P, int G, const LaunchCfg& L);
+void u1_launch_contract(const DevState& S, const Plan& P, int G, const LaunchCfg& L);
+cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchCfg& L);
+void u1_launch_select_scatter(const DevState& S, const Plan& P, int G, int chi, double cutoff, const LaunchCfg& L);
+void u1_launch_expect_n(const DevState& S, double* out_dev, const LaunchCfg& L);
+void u1_launch_entropy(const DevState& S, double* out_dev, const LaunchCfg& L);
+void u1_launch_product_state(const DevState& S, const int* occ_dev, const LaunchCfg& L);
+void u1_launch_gamoff(const DevState& S, int site, const LaunchCfg& L);
+cudaError_t u1_svd_configure(int* grid, int* smem_bytes, int sms);

@@ -1,0 +1,123 @@
+// plan.cu — step a1: sector enumeration and offsets ("a subset of bonds ... that satisfy
+// the conditions on the three charges"; L121: 0 <= c^[k] <= N; Eq.16's deltas bound the occupations
+// by d-1).  Integer only, one CTA, no host round trip: everything later kernels need to find their
+// work (Theta offsets, tile lists, Jacobi item lists) is produced here from the three bond tables.
+#include "common.cuh"
+
+#define PLAN_THREADS 1024
+
+// Exclusive scan of f(0..L-1) into out[0..L] (out[L] = total) by one CTA.
+template <typename T, typename F>
+__device__ void block_excl_scan(F f, T* out, int L, T* sh /*[PLAN_THREADS]*/) {
+  const int t = threadIdx.x;
+  const int per = (L + PLAN_THREADS - 1) / PLAN_THREADS;
+  const int lo = min(L, t * per), hi = min(L, lo + per);
+  T sum = 0;
+  for (int i = lo; i < hi; ++i) sum += f(i);
+  sh[t] = sum;
+  __syncthreads();
+  for (int off = 1; off < PLAN_THREADS; off <<= 1) {  // Hillis-Steele inclusive scan
+    T v = (t >= off) ? sh[t - off] : (T)0;
+    __syncthreads();
+    sh[t] += v;
+    __syncthreads();
+  }
+  T run = sh[t] - sum;
+  for (int i = lo; i < hi; ++i) { T v = f(i); out[i] = run; run += v; }
+  if (t == PLAN_THREADS - 1) out[L] = sh[t];
+  __syncthreads();
+}
+
+__global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, int G, long long smem_elems) {
+  __shared__ long long shl[PLAN_THREADS];
+  __shared__ int shi[PLAN_THREADS];
+  __shared__ int shmax;
+  const int NC = S.NC, d = S.d, E = G * NC, t = threadIdx.x;
+  if (t == 0) shmax = 0;
+  // (i)-(iii) rows(c), cols(c) of every candidate centre charge
+  for (int e = t; e < E; e += PLAN_THREADS) {
+    const int g = e / NC, c = e % NC, s = P.site[g];
+    const int* nL = S.nb + (long long)s * NC;
+    const int* nR = S.nb + (long long)(s + 2) * NC;
+    int r = 0, q = 0;
+    for (int i = 0; i < d; ++i) {
+      if (c + i <= S.N) r += nL[c + i];
+      if (c - i >= 0) q += nR[c - i];
+    }
+    if (r == 0 || q == 0) r = q = 0;
+    P.rows[e] = r;
+    P.cols[e] = q;
+    P.keep[e] = 0;
+  }
+  __syncthreads();
+  // Theta / Jacobi workspace offsets: stacked (m+n) x n column-major, m = max(rows, cols), n = min
+  block_excl_scan<long long>(
+      [&](int e) { long long r = P.rows[e], q = P.cols[e]; long long m = max(r, q), n = min(r, q); return (m + n) * n; },
+      P.goff, E, shl);
+  if (t == 0 && P.goff[E] > P.wcap) atomicExch(S.err, U1_ERR_WORKSPACE);
+  block_excl_scan<int>([&](int e) { return min(P.rows[e], P.cols[e]); }, P.svoff, E, shi);
+  if (t == 0 && P.svoff[E] > P.poolcap) atomicExch(S.err, U1_ERR_WORKSPACE);
+  // (iv) a2 tile list over (e, i, j): block (c_l = c+i, c_r = c-j) of Theta(c)
+  const int dd = d * d;
+  block_excl_scan<int>(
+      [&](int f) {
+        const int e = f / dd, i = (f / d) % d, j = f % d;
+        if (P.rows[e] == 0) return 0;
+        const int g = e / NC, c = e % NC, s = P.site[g];
+        if (c + i > S.N || c - j < 0) return 0;
+        const int nl = S.nb[(long long)s * NC + c + i], nr = S.nb[(long long)(s + 2) * NC + c - j];
+        return u1_ceil_div(nl, U1_TILE) * u1_ceil_div(nr, U1_TILE);
+      },
+      P.t2pref, E * dd, shi);
+  // a5 tile list over (e, part): V rows x n, W n x cols
+  block_excl_scan<int>(
+      [&](int f) {
+        const int e = f >> 1;
+        const int r = P.rows[e], q = P.cols[e], n = min(r, q);
+        if (n == 0) return 0;
+        return (f & 1) ? u1_ceil_div(n, U1_TILE) * u1_ceil_div(q, U1_TILE) : u1_ceil_div(r, U1_TILE) * u1_ceil_div(n, U1_TILE);
+      },
+      P.t5pref, E * 2, shi);
+  // Jacobi block list and item lists
+  auto panels = [&](int e) {
+    const int r = P.rows[e], q = P.cols[e], n = min(r, q), m = max(r, q);
+    if (n == 0) return 0;
+    int in_smem;
+    const int b = u1_panel_width(m + n, n, smem_elems, &in_smem);
+    return u1_ceil_div(n, b);
+  };
+  block_excl_scan<int>([&](int e) { return min(P.rows[e], P.cols[e]) > 0 ? 1 : 0; }, P.tmpa, E, shi);
+  for (int e = t; e < E; e += PLAN_THREADS)
+    if (min(P.rows[e], P.cols[e]) > 0) P.blk[P.tmpa[e]] = e;
+  if (t == 0) P.cnt[0] = P.tmpa[E];
+  __syncthreads();
+  block_excl_scan<int>([&](int e) { int p = panels(e); return p > 1 ? (p + 1) / 2 : 0; }, P.tmpa, E, shi);
+  block_excl_scan<int>([&](int e) { return panels(e); }, P.tmpb, E, shi);
+  if (t == 0) {
+    P.cnt[1] = P.tmpa[E];
+    P.cnt[2] = P.tmpb[E];
+    P.cnt[4] = P.t2pref[E * dd];
+    P.cnt[5] = P.t5pref[E * 2];
+    if (P.tmpa[E] > P.itemcap || P.tmpb[E] > P.itemcap) atomicExch(S.err, U1_ERR_WORKSPACE);
+  }
+  __syncthreads();
+  const bool ok = P.tmpa[E] <= P.itemcap && P.tmpb[E] <= P.itemcap;
+  int mymax = 0;
+  for (int e = t; e < E; e += PLAN_THREADS) {
+    const int p = panels(e);
+    if (p == 0 || !ok) continue;
+    mymax = max(mymax, p + (p & 1));
+    const int np = p > 1 ? (p + 1) / 2 : 0;
+    for (int k = 0; k < np; ++k) { P.pitem_e[P.tmpa[e] + k] = e; P.pitem_k[P.tmpa[e] + k] = k; }
+    for (int k = 0; k < p; ++k) { P.iitem_e[P.tmpb[e] + k] = e; P.iitem_p[P.tmpb[e] + k] = k; }
+  }
+  atomicMax(&shmax, mymax);
+  for (int i = t; i < E * U1_MAXSWEEP; i += PLAN_THREADS) P.flags[i] = 0;
+  __syncthreads();
+  if (t == 0) P.cnt[3] = shmax;
+}
+
+void u1_launch_plan(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
+  plan_kernel<<<1, PLAN_THREADS, 0, L.stream>>>(S, P, G, (long long)L.svd_smem / (long long)sizeof(cplx));
+  ++*L.launches;
+}

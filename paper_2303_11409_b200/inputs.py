@@ -197,3 +197,58 @@ def small_variant(w: Workload, M: int, N: int, chi: int, columns: int, occ=None)
     assert sum(occ) == N and len(occ) == M
     return Workload(w.index, w.name + f"-small-M{M}", M, w.d, N, chi, w.cutoff, tuple(occ), w.family,
                     columns, w.delta, w.dt)
+
+
+# --------------------------------------------------------------------------------------
+# synthetic saturated-bond state for per-gate parity tests and the per-gate microbenchmark
+# (parabolic sector profile, random blocks, geometric lambda inside a sector)
+# --------------------------------------------------------------------------------------
+def parabolic_profile(chi: int, R: int) -> List[int]:
+    """R sector sizes ~ 1 - ((x - x0)/((R+1)/2))^2, each >= 1, summing exactly to chi."""
+    x0 = (R - 1) / 2.0
+    w = np.array([1.0 - ((x - x0) / ((R + 1) / 2.0)) ** 2 for x in range(R)])
+    n = np.maximum(1, np.floor(w / w.sum() * chi).astype(int))
+    i = 0
+    while n.sum() < chi:
+        n[(R // 2 + i) % R] += 1
+        i += 1
+    while n.sum() > chi:
+        j = int(np.argmax(n))
+        n[j] -= 1
+    return [int(v) for v in n]
+
+
+def synthetic_gate_state(d: int, chi: int, R: int, seed: int, decay: float = 0.97):
+    """Random three-bond neighbourhood for one gate on sites (2, 3) of a short chain (M >= 6).
+
+    Returns (M, N, site, lam, gam): lam[k] = {c: descending positive vector} for bonds 2, 3, 4;
+    gam[s] = {(cl, cr): random complex block} for sites 2, 3.  Bond k's sector charges are
+    c0_k .. c0_k + R - 1 with c0 dropping by (d - 1) // 2 + (d % 2 == 0) per bond, so that every
+    occupation 0..d-1 occurs.  No arithmetic of the method is done here: the blocks are plain
+    random numbers (the update is defined for any Gamma and any positive lambda).
+    """
+    rng = np.random.default_rng(seed)
+    site = 2
+    step = max(1, d // 2)
+    N = R + 4 * step + 2
+    M = max(6, -(-N // (d - 1)) + 1)
+    prof = parabolic_profile(chi, R)
+    lam, gam = {}, {}
+    for k in (2, 3, 4):
+        c0 = N - 2 - (k - 1) * step - R // 2 + 1
+        c0 = max(0, c0)
+        lk = {}
+        for x, n in enumerate(prof):
+            v = np.sort(rng.uniform(0.5, 1.0, n) * decay ** np.arange(n))[::-1]
+            lk[c0 + x] = v
+        tot = math.sqrt(sum(float(np.sum(v ** 2)) for v in lk.values()))
+        lam[k] = {c: v / tot for c, v in lk.items()}
+    for s in (2, 3):
+        gs = {}
+        for cl, vl in lam[s].items():
+            for cr, vr in lam[s + 1].items():
+                if 0 <= cl - cr <= d - 1:
+                    nl, nr = len(vl), len(vr)
+                    gs[(cl, cr)] = (rng.standard_normal((nl, nr)) + 1j * rng.standard_normal((nl, nr))) / math.sqrt(nl + nr)
+        gam[s] = gs
+    return M, N, site, lam, gam

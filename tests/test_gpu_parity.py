@@ -1,0 +1,235 @@
+"""`-m gpu` parity tests: the CUDA path (through the C ABI, via the ctypes binding) against the
+CPU oracle on the same seeded inputs.  Tolerances are BASELINE.json's: 1e-10 relative (normwise,
+reading S17) for singular values and reconstructed Theta / amplitudes, 1e-9 for <n_k> and bond
+entropies; sector enumeration, offsets and kept counts bit-exact away from near-ties (S8)."""
+import numpy as np
+import pytest
+
+import statevector_ref as sv
+from gpu_helpers import compare_gate, gpu_to_oracle, make_gpu, oracle_to_gpu
+from paper_2303_11409_b200 import inputs
+from u1mps_oracle import U1MPS as Oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def run_both(w, columns=None):
+    ora = Oracle.product_state(w.M, w.d, w.N, w.chi, w.occ)
+    gpu = make_gpu(w.M, w.d, w.N, w.chi)
+    gpu.set_product_state(w.occ)
+    for sites, us in inputs.gate_columns(w, columns):
+        for g, s in enumerate(sites):
+            ora.apply_gate(int(s), us[g], cutoff=w.cutoff)
+        gpu.apply_gate_column(sites, us, cutoff=w.cutoff)
+    return ora, gpu
+
+
+def assert_observables(ora, gpu, tol=1e-9):
+    assert [int(x) for x in gpu.bond_dims()] == [ora.bond_dim(k) for k in range(ora.M + 1)]
+    for k in range(ora.M + 1):
+        assert dict(gpu.bond_info(k)) == {c: len(v) for c, v in ora.lam[k].items()}
+    n_gpu = gpu.expect_n_all()
+    n_ora = np.array([ora.expect_n(s) for s in range(ora.M)])
+    assert np.max(np.abs(n_gpu - n_ora)) <= tol
+    s_gpu = gpu.bond_entropy_all()
+    s_ora = np.array([ora.bond_entropy(k) for k in range(ora.M + 1)])
+    assert np.max(np.abs(s_gpu - s_ora)) <= tol
+    assert abs(gpu.log_norm() - ora.log_norm) <= tol
+    assert abs(gpu.norm2() - ora.norm2()) <= tol
+    assert abs(gpu.last_stats()["discarded"] - ora.discarded_total) <= tol
+
+
+# ------------------------------------------------------------------ config 1: full, vs the 2^16 state vector
+def test_config1_state_vector():
+    w = inputs.WORKLOADS[1]
+    ora, gpu = run_both(w)
+    assert_observables(ora, gpu)
+    vec = sv.product_vector(w.occ, w.d)
+    for sites, us in inputs.gate_columns(w):
+        for g, s in enumerate(sites):
+            vec = sv.apply_two_site(vec, w.M, w.d, int(s), us[g])
+    amp = gpu_to_oracle(gpu).amplitudes()
+    # gauge: the global phase is fixed (no gauge freedom in amplitudes); compare directly
+    assert np.max(np.abs(amp - vec)) <= 1e-10
+    assert np.count_nonzero(np.abs(vec) > 1e-14) <= 12870
+    assert abs(gpu.norm2() - 1.0) <= 1e-10
+    assert abs(np.sum(gpu.expect_n_all()) - w.N) <= 1e-9
+    assert gpu.last_stats()["converged"]
+
+
+# ------------------------------------------------------------------ free-running trajectories (reduced chains)
+@pytest.mark.parametrize("idx,M,N,chi,cols", [
+    (2, 16, 8, 24, 12),     # truncating (exact rank is 70 at the centre)
+    (3, 20, 10, 48, 16),    # XXZ TEBD, near-identity gates
+    (4, 8, 4, 40, 8),       # beam splitters, d = 5
+    (5, 10, 5, 32, 10),     # beam splitters, d = 4, alternating input
+])
+def test_free_running_small(idx, M, N, chi, cols):
+    w = inputs.small_variant(inputs.WORKLOADS[idx], M=M, N=N, chi=chi, columns=cols)
+    ora, gpu = run_both(w)
+    assert_observables(ora, gpu)
+    if w.d ** w.M <= 2 ** 22:
+        a_gpu = gpu_to_oracle(gpu).amplitudes()
+        a_ora = ora.amplitudes()
+        assert np.max(np.abs(a_gpu - a_ora)) <= 1e-10
+
+
+# ------------------------------------------------------------------ teacher-forced, every gate
+@pytest.mark.parametrize("idx,M,N,chi,cols", [
+    (2, 12, 6, 20, 10),
+    (4, 8, 4, 30, 8),
+    (5, 8, 4, 24, 8),
+])
+def test_teacher_forced_every_gate(idx, M, N, chi, cols):
+    w = inputs.small_variant(inputs.WORKLOADS[idx], M=M, N=N, chi=chi, columns=cols)
+    ora = Oracle.product_state(w.M, w.d, w.N, w.chi, w.occ)
+    gpu = make_gpu(w.M, w.d, w.N, w.chi)
+    gpu.set_product_state(w.occ)
+    ties = 0
+    for sites, us in inputs.gate_columns(w):
+        for g, s in enumerate(sites):
+            s = int(s)
+            oracle_to_gpu(ora, gpu, bonds=[s, s + 1, s + 2], sites=[s, s + 1])
+            _, tie = compare_gate(gpu, ora, s, us[g], w.chi, w.cutoff)
+            ties += tie
+    assert ties <= 2
+
+
+# ------------------------------------------------------------------ synthetic saturated bonds: several tiles, ragged tails,
+# all three Jacobi paths (two panels in smem with b=16, b=8, and in place through L2)
+@pytest.mark.parametrize("d,chi,R,keep_chi", [
+    (2, 96, 4, 64),       # sectors ~ 24..48 wide: single/multi panel, b = 16
+    (2, 333, 5, 200),     # ragged: blocks ~ 130 x 150, m + n <= 400 -> b = 16 in smem
+    (2, 700, 4, 512),     # m + n ~ 700 -> b = 8 in smem
+    (2, 1024, 3, 1024),   # m + n > 800 -> in-place path
+    (4, 256, 6, 256),     # d = 4: rows(c) spans 4 left sectors
+    (5, 180, 7, 100),     # d = 5
+])
+def test_synthetic_gate(d, chi, R, keep_chi):
+    M, N, s, lam, gam = inputs.synthetic_gate_state(d, chi, R, seed=1234 + chi)
+    rng = np.random.default_rng(99 + chi)
+    U = inputs.random_u1_gate(rng, d, unitary=(d == 2))
+    occ = [0] * M
+    left = N
+    for i in range(M):
+        occ[i] = min(d - 1, left)
+        left -= occ[i]
+    assert left == 0
+    ora = Oracle.product_state(M, d, N, chi, occ)
+    for k in (2, 3, 4):
+        ora.sectors[k] = sorted(lam[k])
+        ora.lam[k] = lam[k]
+    for st in (2, 3):
+        ora.gam[st] = gam[st]
+    gpu = make_gpu(M, d, N, chi)
+    gpu.set_product_state(occ)
+    oracle_to_gpu(ora, gpu, bonds=[2, 3, 4], sites=[2, 3])
+    rec, tie = compare_gate(gpu, ora, s, U, keep_chi, 1e-12)
+    assert not tie
+    st = gpu.last_stats()
+    assert st["converged"] and st["sweeps"] < 40
+    # a5: the new Gammas reproduce the oracle's truncated Theta (gauge-invariant, reading S16):
+    # lamL Gamma~[s] lam~ Gamma~[s+1] lamR == V_kept sigma_kept W_kept / sqrt(w)
+    g_s, g_s1 = gpu.export_site(s), gpu.export_site(s + 1)
+    lam_new = gpu.export_bond(s + 1)
+    w = rec.weight_kept
+    fro = np.sqrt(rec.weight_all)
+    for c, kc in rec.keep.items():
+        if kc == 0:
+            continue
+        want = (rec.V[c][:, :kc] * rec.sigma[c][None, :kc]) @ rec.W[c][:kc, :] / np.sqrt(w)
+        got = np.zeros_like(want)
+        for cl, ro, nr in rec.rows[c]:
+            for cr, co, ncol in rec.cols[c]:
+                blk = (lam[s][cl][:, None] * g_s[(cl, c)] * lam_new[c][None, :]) @ (g_s1[(c, cr)] * lam[s + 2][cr][None, :])
+                got[ro:ro + nr, co:co + ncol] = blk
+        assert np.linalg.norm(got - want) <= 1e-10 * fro / np.sqrt(w), c
+
+
+# ------------------------------------------------------------------ API semantics and edge cases
+def test_column_equals_gate_by_gate():
+    w = inputs.small_variant(inputs.WORKLOADS[2], M=12, N=6, chi=16, columns=8)
+    a = make_gpu(w.M, w.d, w.N, w.chi)
+    b = make_gpu(w.M, w.d, w.N, w.chi)
+    a.set_product_state(w.occ)
+    b.set_product_state(w.occ)
+    for sites, us in inputs.gate_columns(w):
+        a.apply_gate_column(sites, us, cutoff=w.cutoff)
+        for g, s in enumerate(sites):
+            b.apply_two_site_gate(int(s), us[g])
+            b.truncate(int(s), w.chi, w.cutoff)
+    assert np.array_equal(a.bond_dims(), b.bond_dims())
+    assert np.array_equal(a.expect_n_all(), b.expect_n_all())       # same kernels, same order: bit-identical
+    assert np.array_equal(a.bond_entropy_all(), b.bond_entropy_all())
+
+
+def test_device_resident_gates():
+    import torch
+    w = inputs.small_variant(inputs.WORKLOADS[2], M=10, N=5, chi=16, columns=6)
+    a = make_gpu(w.M, w.d, w.N, w.chi)
+    b = make_gpu(w.M, w.d, w.N, w.chi)
+    a.set_product_state(w.occ)
+    b.set_product_state(w.occ)
+    for sites, us in inputs.gate_columns(w):
+        a.apply_gate_column(sites, us, cutoff=w.cutoff)
+        b.apply_gate_column(sites, torch.from_numpy(us).cuda(), cutoff=w.cutoff)
+    assert np.array_equal(a.expect_n_all(), b.expect_n_all())
+
+
+def test_identity_and_swap_gates():
+    d, M, N = 3, 6, 5
+    occ = [2, 0, 1, 0, 2, 0]
+    gpu = make_gpu(M, d, N, 8)
+    gpu.set_product_state(occ)
+    gpu.apply_and_truncate(1, np.eye(d * d, dtype=np.complex128))
+    assert np.allclose(gpu.expect_n_all(), occ, atol=1e-14)
+    gpu.apply_and_truncate(0, inputs.swap_gate(d))          # |2,0> -> |0,2>
+    gpu.apply_and_truncate(3, inputs.swap_gate(d))          # |0,2> -> |2,0>
+    assert np.allclose(gpu.expect_n_all(), [0, 2, 1, 2, 0, 0], atol=1e-14)
+    assert list(gpu.bond_dims()) == [1] * (M + 1)
+    assert abs(gpu.norm2() - 1.0) < 1e-14
+
+
+def test_chi_one_truncation_and_nonunitary_gate():
+    w = inputs.small_variant(inputs.WORKLOADS[5], M=6, N=3, chi=8, columns=4)
+    ora = Oracle.product_state(w.M, w.d, w.N, w.chi, w.occ)
+    gpu = make_gpu(w.M, w.d, w.N, w.chi)
+    gpu.set_product_state(w.occ)
+    rng = np.random.default_rng(5)
+    for t in range(4):
+        for s in inputs.column_sites(w.M, t):
+            U = inputs.random_u1_gate(rng, w.d, unitary=False)      # Ginibre blocks: not unitary (S13)
+            chi = 1 if (t == 3) else w.chi
+            ora.apply_gate(s, U, chi=chi, cutoff=1e-12)
+            gpu.apply_and_truncate(s, U, chi=chi, cutoff=1e-12)
+    assert_observables(ora, gpu)
+    assert max(gpu.bond_dims()) <= 8
+
+
+def test_error_codes():
+    from paper_2303_11409_b200.binding import U1MPSError
+    gpu = make_gpu(6, 2, 3, 8)
+    with pytest.raises(U1MPSError) as e:
+        gpu.set_product_state([1, 1, 1, 1, 0, 0])       # sum != N
+    assert e.value.code == -1
+    gpu.set_product_state([1, 0, 1, 0, 1, 0])
+    bad = np.zeros((4, 4), dtype=np.complex128)
+    bad[0, 3] = 1.0                                       # |11> -> |00| violates charge conservation
+    with pytest.raises(U1MPSError) as e:
+        gpu.apply_two_site_gate(0, bad)
+    assert e.value.code == -2
+    with pytest.raises(U1MPSError) as e:
+        gpu.apply_two_site_gate(5, np.eye(4, dtype=np.complex128))   # site out of range
+    assert e.value.code == -1
+    gpu.apply_two_site_gate(2, np.eye(4, dtype=np.complex128))
+    with pytest.raises(U1MPSError) as e:
+        gpu.apply_two_site_gate(0, np.eye(4, dtype=np.complex128))   # staged
+    assert e.value.code == -3
+    with pytest.raises(U1MPSError) as e:
+        gpu.truncate(1, 8, 1e-12)                         # wrong bond
+    assert e.value.code == -3
+    gpu.truncate(2, 8, 1e-12)
+    with pytest.raises(U1MPSError) as e:
+        gpu.apply_gate_column([0, 1], np.stack([np.eye(4, dtype=np.complex128)] * 2))   # overlapping gates
+    assert e.value.code == -1
+    assert np.allclose(gpu.expect_n_all(), [1, 0, 1, 0, 1, 0])
