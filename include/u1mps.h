@@ -128,6 +128,14 @@ int u1mps_export_staged_theta(u1mps_t* h, int c, void* theta_host, size_t cap);
  * r = min(rows, cols), row-major.  Any of the three pointers may be NULL. */
 int u1mps_export_staged_svd(u1mps_t* h, int c, void* V_host, double* sigma_host, void* W_host);
 
+/* Per-kernel device timing (for bench.py's roofline): while enabled, every kernel launch of the handle is
+ * bracketed by CUDA events on the handle's stream; u1mps_profile_read [sync] sums the elapsed times (ms) and
+ * launch counts per stage since the last read / enable into HOST arrays of U1MPS_NSTAGE entries and resets. */
+#define U1MPS_NSTAGE 8
+int u1mps_profile_enable(u1mps_t* h, int on);
+int u1mps_profile_read(u1mps_t* h, double* ms_host, long long* launches_host);
+const char* u1mps_stage_name(int stage); /* "a1_plan", "a2_contract", ... ; "" if out of range */
+
 /* Number of kernels this handle has launched since create (for bench.py's gpu_launches). */
 int u1mps_launch_count(u1mps_t* h, long long* out_host);
 

@@ -21,8 +21,10 @@ EXPORTS = [
     "u1mps_expect_n", "u1mps_expect_n_all", "u1mps_bond_entropy", "u1mps_bond_entropy_all", "u1mps_bond_info",
     "u1mps_bond_dims", "u1mps_last_stats", "u1mps_export_bond", "u1mps_export_site", "u1mps_import_bond",
     "u1mps_import_site", "u1mps_set_log_norm", "u1mps_staged_info", "u1mps_export_staged_theta",
-    "u1mps_export_staged_svd", "u1mps_launch_count",
+    "u1mps_export_staged_svd", "u1mps_launch_count", "u1mps_profile_enable", "u1mps_profile_read",
+    "u1mps_stage_name",
 ]
+NSTAGE = 8
 
 ENOCONV = -6
 
@@ -78,8 +80,12 @@ def load_library() -> C.CDLL:
     lib.u1mps_export_staged_theta.argtypes = [vp, C.c_int, vp, C.c_size_t]
     lib.u1mps_export_staged_svd.argtypes = [vp, C.c_int, vp, dp, vp]
     lib.u1mps_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
+    lib.u1mps_profile_enable.argtypes = [vp, C.c_int]
+    lib.u1mps_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+    lib.u1mps_stage_name.restype = C.c_char_p
+    lib.u1mps_stage_name.argtypes = [C.c_int]
     for name in EXPORTS:
-        if name not in ("u1mps_strerror", "u1mps_version", "u1mps_workspace_bytes"):
+        if name not in ("u1mps_strerror", "u1mps_version", "u1mps_workspace_bytes", "u1mps_stage_name"):
             getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -223,6 +229,16 @@ class U1MPS:
         dw, kept, sw = C.c_double(), C.c_int(), C.c_int()
         code = self._ck(self.lib.u1mps_last_stats(self.h, C.byref(dw), C.byref(kept), C.byref(sw)), allow=(ENOCONV,))
         return {"discarded": dw.value, "kept": kept.value, "sweeps": sw.value, "converged": code == 0}
+
+    def profile_enable(self, on: bool = True):
+        self._ck(self.lib.u1mps_profile_enable(self.h, 1 if on else 0))
+
+    def profile_read(self) -> Dict[str, Tuple[float, int]]:
+        """{stage name: (summed device ms, launches)} since the last read."""
+        ms = np.zeros(NSTAGE)
+        n = np.zeros(NSTAGE, np.int64)
+        self._ck(self.lib.u1mps_profile_read(self.h, _ptr(ms, C.POINTER(C.c_double)), _ptr(n, C.POINTER(C.c_longlong))))
+        return {self.lib.u1mps_stage_name(s).decode(): (float(ms[s]), int(n[s])) for s in range(NSTAGE)}
 
     def launch_count(self) -> int:
         v = C.c_longlong()

@@ -71,6 +71,7 @@ struct u1mps {
   int Gmax;
   cudaStream_t stream;
   LaunchCfg L;
+  Prof prof;
   long long launches;
   std::vector<long long> Dh;  // host upper bounds of the bond dimensions
   Stage stage;
@@ -228,7 +229,7 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
   if (e == cudaSuccess) e = cudaMemsetAsync(S.err, 0, 8 * 4, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(S.scal, 0, 8 * 8, h->stream);
   if (e != cudaSuccess) { delete h; return U1MPS_ECUDA; }
-  h->L.sms = sms; h->L.svd_grid = grid; h->L.svd_smem = smem; h->L.stream = h->stream; h->L.launches = &h->launches;
+  h->L.sms = sms; h->L.svd_grid = grid; h->L.svd_smem = smem; h->L.stream = h->stream; h->L.launches = &h->launches; h->L.prof = &h->prof;
   *out = h;
   return U1MPS_OK;
 }
@@ -236,6 +237,7 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
 int u1mps_destroy(u1mps_t* h) {
   if (!h) return U1MPS_EINVAL;
   cudaStreamSynchronize(h->stream);
+  h->prof.destroy();
   delete h;
   return U1MPS_OK;
 }
@@ -615,6 +617,34 @@ int u1mps_export_staged_svd(u1mps_t* h, int c, void* V, double* sigma, void* Wou
       }
   }
   return check_device_flags(h);
+}
+
+int u1mps_profile_enable(u1mps_t* h, int on) {
+  if (!h) return U1MPS_EINVAL;
+  CK(cudaStreamSynchronize(h->stream));
+  h->prof.used = 0;
+  h->prof.on = on != 0;
+  return U1MPS_OK;
+}
+
+int u1mps_profile_read(u1mps_t* h, double* ms, long long* launches) {
+  if (!h || !ms || !launches) return U1MPS_EINVAL;
+  CK(cudaStreamSynchronize(h->stream));
+  for (int s = 0; s < U1MPS_NSTAGE; ++s) { ms[s] = 0.0; launches[s] = 0; }
+  for (size_t i = 0; i < h->prof.used; ++i) {
+    float t = 0.f;
+    CK(cudaEventElapsedTime(&t, h->prof.pool[2 * i], h->prof.pool[2 * i + 1]));
+    ms[h->prof.stage[i]] += t;
+    ++launches[h->prof.stage[i]];
+  }
+  h->prof.used = 0;
+  return U1MPS_OK;
+}
+
+const char* u1mps_stage_name(int stage) {
+  static const char* names[U1MPS_NSTAGE] = {"a1_plan", "a2_contract", "a2_identity", "a3_svd", "a3_sigma_sort",
+                                            "a4_select", "a5_scatter", "a6_readout"};
+  return (stage >= 0 && stage < U1MPS_NSTAGE) ? names[stage] : "";
 }
 
 int u1mps_launch_count(u1mps_t* h, long long* out) {

@@ -69,8 +69,35 @@ __host__ __device__ inline int u1_panel_width(int mt, int n, long long smem_elem
   return U1_PANEL;
 }
 
+// Optional per-kernel timing (u1mps_profile_*): CUDA events recorded on the handle's stream around
+// every launch of a stage; summed when read.  Host side only.
+enum { U1_ST_PLAN = 0, U1_ST_CONTRACT, U1_ST_IDENTITY, U1_ST_SVD, U1_ST_SORT, U1_ST_SELECT, U1_ST_SCATTER, U1_ST_READOUT, U1_NSTAGE };
+#include <vector>
+struct Prof {
+  bool on = false;
+  std::vector<cudaEvent_t> pool;     // begin/end pairs, reused
+  std::vector<int> stage;            // stage of pair i
+  size_t used = 0;                   // pairs in flight
+  void begin(int st, cudaStream_t s) {
+    if (!on) return;
+    if (used == stage.size()) {
+      cudaEvent_t a, b;
+      if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { on = false; return; }
+      pool.push_back(a); pool.push_back(b); stage.push_back(st);
+    }
+    stage[used] = st;
+    cudaEventRecord(pool[2 * used], s);
+  }
+  void end(cudaStream_t s) {
+    if (!on) return;
+    cudaEventRecord(pool[2 * used + 1], s);
+    ++used;
+  }
+  void destroy() { for (cudaEvent_t e : pool) cudaEventDestroy(e); pool.clear(); stage.clear(); used = 0; }
+};
+
 // Host-side launchers (one per kernel file).  `stream` is the handle's stream.
-struct LaunchCfg { int sms; int svd_grid; int svd_smem; cudaStream_t stream; long long* launches; };
+struct LaunchCfg { int sms; int svd_grid; int svd_smem; cudaStream_t stream; long long* launches; Prof* prof; };
 
 void u1_launch_plan(const DevState& S, const Plan& P, int G, const LaunchCfg& L);
 void u1_launch_contract(const DevState& S, const Plan& P, int G, const LaunchCfg& L);

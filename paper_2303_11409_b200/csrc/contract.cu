@@ -132,7 +132,11 @@ __global__ void identity_kernel(Plan P) {
 }
 
 void u1_launch_contract(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
+  L.prof->begin(U1_ST_CONTRACT, L.stream);
   contract_kernel<<<L.sms * 4, CT_THREADS, 0, L.stream>>>(S, P, G);
+  L.prof->end(L.stream);
+  L.prof->begin(U1_ST_IDENTITY, L.stream);
   identity_kernel<<<L.sms * 2, 256, 0, L.stream>>>(P);
+  L.prof->end(L.stream);
   *L.launches += 2;
 }

@@ -118,6 +118,8 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
 }
 
 void u1_launch_plan(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
+  L.prof->begin(U1_ST_PLAN, L.stream);
   plan_kernel<<<1, PLAN_THREADS, 0, L.stream>>>(S, P, G, (long long)L.svd_smem / (long long)sizeof(cplx));
+  L.prof->end(L.stream);
   ++*L.launches;
 }

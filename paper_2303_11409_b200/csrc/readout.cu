@@ -108,11 +108,15 @@ __global__ void product_state_kernel(DevState S, const int* occ) {
 }
 
 void u1_launch_expect_n(const DevState& S, double* out_dev, const LaunchCfg& L) {
+  L.prof->begin(U1_ST_READOUT, L.stream);
   expect_n_kernel<<<S.M, RD_THREADS, 0, L.stream>>>(S, out_dev);
+  L.prof->end(L.stream);
   ++*L.launches;
 }
 void u1_launch_entropy(const DevState& S, double* out_dev, const LaunchCfg& L) {
+  L.prof->begin(U1_ST_READOUT, L.stream);
   entropy_kernel<<<S.M + 1, RD_THREADS, 0, L.stream>>>(S, out_dev);
+  L.prof->end(L.stream);
   ++*L.launches;
 }
 void u1_launch_product_state(const DevState& S, const int* occ_dev, const LaunchCfg& L) {

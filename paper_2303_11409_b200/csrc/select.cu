@@ -202,7 +202,11 @@ __global__ void __launch_bounds__(SC_THREADS) scatter_kernel(DevState S, Plan P,
 
 void u1_launch_select_scatter(const DevState& S, const Plan& P, int G, int chi, double cutoff, const LaunchCfg& L) {
   int* counter = P.cnt + 7;
+  L.prof->begin(U1_ST_SELECT, L.stream);
   select_kernel<<<G, SEL_THREADS, S.NC * sizeof(int), L.stream>>>(S, P, G, chi, cutoff, counter, P.gate_w);
+  L.prof->end(L.stream);
+  L.prof->begin(U1_ST_SCATTER, L.stream);
   scatter_kernel<<<L.sms * 4, SC_THREADS, 0, L.stream>>>(S, P, G);
+  L.prof->end(L.stream);
   *L.launches += 2;
 }

@@ -261,10 +261,14 @@ cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchC
   long long smem_elems = (long long)L.svd_smem / (long long)sizeof(cplx);
   DevState s = S; Plan p = P; int g = G;
   void* args[] = {&s, &p, &g, &smem_elems};
+  L.prof->begin(U1_ST_SVD, L.stream);
   cudaError_t err = cudaLaunchCooperativeKernel((void*)svd_kernel, dim3(L.svd_grid), dim3(U1_SVD_THREADS), args,
                                                 (size_t)L.svd_smem, L.stream);
+  L.prof->end(L.stream);
   if (err != cudaSuccess) return err;
+  L.prof->begin(U1_ST_SORT, L.stream);
   sigma_sort_kernel<<<L.sms * 2, SORT_THREADS, U1MPS_SORT_MAX * 12, L.stream>>>(P);
+  L.prof->end(L.stream);
   *L.launches += 2;
   return cudaGetLastError();
 }

@@ -55,10 +55,12 @@ def compare_gate(gpu, ora_pre: Oracle, s, U, chi, cutoff, tol_sigma=1e-10, tol_t
         assert [c for c, _, _ in info] == rec.charges
     sig1 = max(float(rec.sigma[c][0]) for c in rec.charges)
     fro = np.sqrt(sum(np.linalg.norm(rec.theta[c]) ** 2 for c in rec.charges))
+    dev = 0.0   # largest observed |sigma_gpu - sigma_oracle| of this gate
     for c, rows, cols in info:
         V, S, W = gpu.export_staged_svd(c, rows, cols)
         assert np.all(np.diff(S) <= 0), "sigma not descending"
         assert np.max(np.abs(S - rec.sigma[c])) <= tol_sigma * sig1, (c, np.max(np.abs(S - rec.sigma[c])), sig1)
+        dev = max(dev, float(np.max(np.abs(S - rec.sigma[c]))))
         recon = (V * S[None, :]) @ W
         assert np.linalg.norm(recon - rec.theta[c]) <= tol_theta * fro, (c, np.linalg.norm(recon - rec.theta[c]), fro)
         # singular vectors of the kept part are orthonormal (V, W isometries, pin P4's basis)
@@ -68,8 +70,12 @@ def compare_gate(gpu, ora_pre: Oracle, s, U, chi, cutoff, tol_sigma=1e-10, tol_t
             assert np.linalg.norm(Vb.conj().T @ Vb - np.eye(Vb.shape[1])) <= 1e-9
             assert np.linalg.norm(Wb @ Wb.conj().T - np.eye(Wb.shape[0])) <= 1e-9
     gpu.truncate(s, chi, cutoff)
-    # a4: kept counts bit-exact unless there is a near-tie at the cut (reading S8)
-    near_tie = (rec.sigma_next > 0 and abs(rec.sigma_chi - rec.sigma_next) <= 1e-10 * sig1) or rec.cutoff_gap <= 1e-10 * sig1
+    # a4: kept counts bit-exact unless there is a near-tie at the cut (reading S8: |sigma_chi - sigma_chi+1|
+    # <= 1e-10 sigma_1).  At the absolute cutoff (S7) the decision sigma > cutoff can only differ if an oracle
+    # sigma lies within the observed GPU/oracle deviation of the cutoff (exact zeros of a rank-deficient
+    # Theta come out ~1e-17 on both sides and are not ties).
+    near_tie = ((rec.sigma_next > 0 and abs(rec.sigma_chi - rec.sigma_next) <= 1e-10 * sig1)
+                or rec.cutoff_gap <= 2.0 * dev)
     got = dict(gpu.bond_info(s + 1))
     want = {c: k for c, k in rec.keep.items() if k > 0}
     if not near_tie:
