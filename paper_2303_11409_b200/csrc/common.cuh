@@ -7,8 +7,9 @@
 typedef double2 cplx;  // complex128, interleaved (x = re, y = im), 16-byte aligned
 
 #define U1_TILE 32         // a2 / a5 tile edge
-#define U1_MAXSWEEP 40     // Jacobi sweep limit
-#define U1_PANEL 16        // max columns per Jacobi panel
+#define U1_MAXSWEEP 30     // Jacobi (outer) sweep limit
+#define U1_PANEL 16        // (item-list sizing unit)
+#define U1_PB 32           // columns per Jacobi panel: a pair step orthogonalises 2*U1_PB = 64 columns
 #define U1_ERR_WORKSPACE 1 // device error flag: plan does not fit the workspace
 #define U1_SVD_THREADS 512
 #define U1MPS_SORT_MAX 4096 // largest sector the in-smem bitonic sort takes (= U1MPS_CHI_MAX) // 16 warps: one per column pair of a panel-pair step
@@ -38,6 +39,8 @@ struct Plan {
   int* t2pref;       // [G*NC*d*d+1] a2 tile prefix over (e, i, j)
   int* t5pref;       // [G*NC*2+1] a5 tile prefix over (e, part)  part 0 = V, 1 = W
   int* blk;          // [G*NC] compact list of entries with n > 0
+  cplx* Q;           // [itemcap * 64*64] pair transforms of the current Jacobi round (column-major 64x64 each)
+  int* pact;         // [itemcap] 1 if the pair item rotated in the current round
   int* pitem_e;      // [cap] Jacobi panel-pair items: entry e
   int* pitem_k;      // [cap] ... pair slot k
   int* iitem_e;      // [cap] intra-panel items: entry e

@@ -79,20 +79,18 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
       },
       P.t5pref, E * 2, shi);
   // Jacobi block list and item lists
-  auto panels = [&](int e) {
-    const int r = P.rows[e], q = P.cols[e], n = min(r, q), m = max(r, q);
-    if (n == 0) return 0;
-    int in_smem;
-    const int b = u1_panel_width(m + n, n, smem_elems, &in_smem);
-    return u1_ceil_div(n, b);
+  auto panels = [&](int e) {  // column panels of U1_PB columns of the Jacobi matrix of entry e
+    const int n = min(P.rows[e], P.cols[e]);
+    return u1_ceil_div(n, U1_PB);
   };
   block_excl_scan<int>([&](int e) { return min(P.rows[e], P.cols[e]) > 0 ? 1 : 0; }, P.tmpa, E, shi);
   for (int e = t; e < E; e += PLAN_THREADS)
     if (min(P.rows[e], P.cols[e]) > 0) P.blk[P.tmpa[e]] = e;
   if (t == 0) P.cnt[0] = P.tmpa[E];
   __syncthreads();
-  block_excl_scan<int>([&](int e) { int p = panels(e); return p > 1 ? (p + 1) / 2 : 0; }, P.tmpa, E, shi);
-  block_excl_scan<int>([&](int e) { return panels(e); }, P.tmpb, E, shi);
+  // pair items: (p+1)/2 panel pairs per round of the round-robin tournament; a single panel is one item
+  block_excl_scan<int>([&](int e) { int p = panels(e); return (p + 1) / 2; }, P.tmpa, E, shi);
+  block_excl_scan<int>([&](int e) { return 0; }, P.tmpb, E, shi);
   if (t == 0) {
     P.cnt[1] = P.tmpa[E];
     P.cnt[2] = P.tmpb[E];
@@ -107,9 +105,8 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
     const int p = panels(e);
     if (p == 0 || !ok) continue;
     mymax = max(mymax, p + (p & 1));
-    const int np = p > 1 ? (p + 1) / 2 : 0;
+    const int np = (p + 1) / 2;
     for (int k = 0; k < np; ++k) { P.pitem_e[P.tmpa[e] + k] = e; P.pitem_k[P.tmpa[e] + k] = k; }
-    for (int k = 0; k < p; ++k) { P.iitem_e[P.tmpb[e] + k] = e; P.iitem_p[P.tmpb[e] + k] = k; }
   }
   atomicMax(&shmax, mymax);
   for (int i = t; i < E * U1_MAXSWEEP; i += PLAN_THREADS) P.flags[i] = 0;
