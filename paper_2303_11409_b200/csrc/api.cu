@@ -45,11 +45,11 @@ Sizes compute_sizes(int M, int d, int N, int chi) {
   add((size_t)M * NC * d * 8);                                   // gamoff
   add(8 * 8); add(8 * 4); add((M + 1) * 8); add(M * 4);          // scal, err, dout, occ
   add(z.Gmax * 4); add((size_t)z.Gmax * d * d * d * d * 16);     // site, U
-  for (int i = 0; i < 6; ++i) add((E + 1) * 4);                  // rows cols keep blk tmpa tmpb
+  for (int i = 0; i < 5; ++i) add((E + 1) * 4);                  // rows cols keep blk tmpa
   add((E + 1) * 8); add((E + 1) * 4);                            // goff svoff
   add((E * d * d + 1) * 4); add((2 * E + 1) * 4);                // t2pref t5pref
   add(8 * 4); add(E * U1_MAXSWEEP * 4); add((size_t)2 * z.Gmax * 8);  // cnt flags gate_w
-  for (int i = 0; i < 4; ++i) add((size_t)z.itemcap * 4);        // item lists
+  for (int i = 0; i < 2; ++i) add((size_t)z.itemcap * 4);        // item lists
   add((size_t)z.poolcap * 4); add((size_t)z.poolcap * 8); add((size_t)z.poolcap * 8);  // perm sv svs
   b = (b + 255) & ~(size_t)255;
   z.fixed = b;
@@ -206,12 +206,11 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
   Plan& P = h->P;
   P.site = A.take<int>(z.Gmax); P.U = A.take<cplx>((size_t)z.Gmax * d * d * d * d);
   P.rows = A.take<int>(E + 1); P.cols = A.take<int>(E + 1); P.keep = A.take<int>(E + 1);
-  P.blk = A.take<int>(E + 1); P.tmpa = A.take<int>(E + 1); P.tmpb = A.take<int>(E + 1);
+  P.blk = A.take<int>(E + 1); P.tmpa = A.take<int>(E + 1);
   P.goff = A.take<long long>(E + 1); P.svoff = A.take<int>(E + 1);
   P.t2pref = A.take<int>(E * d * d + 1); P.t5pref = A.take<int>(2 * E + 1);
   P.cnt = A.take<int>(8); P.flags = A.take<int>(E * U1_MAXSWEEP); P.gate_w = A.take<double>((size_t)2 * z.Gmax);
   P.pitem_e = A.take<int>(z.itemcap); P.pitem_k = A.take<int>(z.itemcap);
-  P.iitem_e = A.take<int>(z.itemcap); P.iitem_p = A.take<int>(z.itemcap);
   P.perm = A.take<int>(z.poolcap); P.sv = A.take<double>(z.poolcap); P.svs = A.take<double>(z.poolcap);
   P.poolcap = z.poolcap; P.itemcap = z.itemcap;
   size_t off = (A.used + 255) & ~(size_t)255;

@@ -9,10 +9,10 @@ typedef double2 cplx;  // complex128, interleaved (x = re, y = im), 16-byte alig
 #define U1_TILE 32         // a2 / a5 tile edge
 #define U1_MAXSWEEP 30     // Jacobi (outer) sweep limit
 #define U1_PANEL 16        // (item-list sizing unit)
-#define U1_PB 32           // columns per Jacobi panel: a pair step orthogonalises 2*U1_PB = 64 columns
+#define U1_PB 16           // columns per Jacobi panel: a pair item orthogonalises 2*U1_PB = 32 columns
 #define U1_ERR_WORKSPACE 1 // device error flag: plan does not fit the workspace
-#define U1_SVD_THREADS 512
-#define U1MPS_SORT_MAX 4096 // largest sector the in-smem bitonic sort takes (= U1MPS_CHI_MAX) // 16 warps: one per column pair of a panel-pair step
+#define U1_SVD_THREADS 256 // 8 warps: DMMA tiles of the Gram / update GEMMs, 16 x 16 two-by-two units of the inner EVD
+#define U1MPS_SORT_MAX 4096 // largest sector the in-smem bitonic sort takes (= U1MPS_CHI_MAX)
 
 // Persistent MPS state (all device pointers into the caller's arena).
 struct DevState {
@@ -39,15 +39,10 @@ struct Plan {
   int* t2pref;       // [G*NC*d*d+1] a2 tile prefix over (e, i, j)
   int* t5pref;       // [G*NC*2+1] a5 tile prefix over (e, part)  part 0 = V, 1 = W
   int* blk;          // [G*NC] compact list of entries with n > 0
-  cplx* Q;           // [itemcap * 64*64] pair transforms of the current Jacobi round (column-major 64x64 each)
-  int* pact;         // [itemcap] 1 if the pair item rotated in the current round
   int* pitem_e;      // [cap] Jacobi panel-pair items: entry e
-  int* pitem_k;      // [cap] ... pair slot k
-  int* iitem_e;      // [cap] intra-panel items: entry e
-  int* iitem_p;      // [cap] ... panel
+  int* pitem_k;      // [cap] ... pair slot k of the round-robin tournament
   int* tmpa;         // [G*NC+1] scratch: pair-item offset per entry
-  int* tmpb;         // [G*NC+1] scratch: intra-item offset per entry
-  int* cnt;          // [8] 0: #blk, 1: #pair items, 2: #intra items, 3: max panels, 4: a2 tiles, 5: a5 tiles, 7: a4 CTA counter
+  int* cnt;          // [8] 0: #blk, 1: #pair items, 3: max panels (even), 4: a2 tiles, 5: a5 tiles, 6: a3 work-queue ticket, 7: a4 CTA counter
   int* flags;        // [G*NC*U1_MAXSWEEP] per entry, per sweep: 1 if any rotation happened
   int* keep;         // [G*NC] kept singular values per entry (a4)
   int* perm;         // [pool] sorted position -> column index
@@ -61,16 +56,6 @@ struct Plan {
 };
 
 __host__ __device__ inline int u1_ceil_div(int a, int b) { return (a + b - 1) / b; }
-
-// Panel width for a block with `mt` = m + n stacked rows and n columns; smem_elems = capacity of the
-// staging buffer in complex elements.  Returns b (columns per panel); *in_smem says whether two
-// panels fit in shared memory.
-__host__ __device__ inline int u1_panel_width(int mt, int n, long long smem_elems, int* in_smem) {
-  if ((long long)mt * 2 * U1_PANEL <= smem_elems) { *in_smem = 1; return U1_PANEL; }
-  if ((long long)mt * U1_PANEL <= smem_elems) { *in_smem = 1; return U1_PANEL / 2; }
-  *in_smem = 0;
-  return U1_PANEL;
-}
 
 // Optional per-kernel timing (u1mps_profile_*): CUDA events recorded on the handle's stream around
 // every launch of a stage; summed when read.  Host side only.

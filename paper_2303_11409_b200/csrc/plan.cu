@@ -28,7 +28,7 @@ __device__ void block_excl_scan(F f, T* out, int L, T* sh /*[PLAN_THREADS]*/) {
   __syncthreads();
 }
 
-__global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, int G, long long smem_elems) {
+__global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, int G) {
   __shared__ long long shl[PLAN_THREADS];
   __shared__ int shi[PLAN_THREADS];
   __shared__ int shmax;
@@ -90,16 +90,15 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
   __syncthreads();
   // pair items: (p+1)/2 panel pairs per round of the round-robin tournament; a single panel is one item
   block_excl_scan<int>([&](int e) { int p = panels(e); return (p + 1) / 2; }, P.tmpa, E, shi);
-  block_excl_scan<int>([&](int e) { return 0; }, P.tmpb, E, shi);
   if (t == 0) {
     P.cnt[1] = P.tmpa[E];
-    P.cnt[2] = P.tmpb[E];
     P.cnt[4] = P.t2pref[E * dd];
     P.cnt[5] = P.t5pref[E * 2];
-    if (P.tmpa[E] > P.itemcap || P.tmpb[E] > P.itemcap) atomicExch(S.err, U1_ERR_WORKSPACE);
+    P.cnt[6] = 0;
+    if (P.tmpa[E] > P.itemcap) atomicExch(S.err, U1_ERR_WORKSPACE);
   }
   __syncthreads();
-  const bool ok = P.tmpa[E] <= P.itemcap && P.tmpb[E] <= P.itemcap;
+  const bool ok = P.tmpa[E] <= P.itemcap;
   int mymax = 0;
   for (int e = t; e < E; e += PLAN_THREADS) {
     const int p = panels(e);
@@ -116,7 +115,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
 
 void u1_launch_plan(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
   L.prof->begin(U1_ST_PLAN, L.stream);
-  plan_kernel<<<1, PLAN_THREADS, 0, L.stream>>>(S, P, G, (long long)L.svd_smem / (long long)sizeof(cplx));
+  plan_kernel<<<1, PLAN_THREADS, 0, L.stream>>>(S, P, G);
   L.prof->end(L.stream);
   ++*L.launches;
 }
