@@ -136,6 +136,12 @@ int u1mps_profile_enable(u1mps_t* h, int on);
 int u1mps_profile_read(u1mps_t* h, double* ms_host, long long* launches_host);
 const char* u1mps_stage_name(int stage); /* "a1_plan", "a2_contract", ... ; "" if out of range */
 
+/* Trace of the LAST a3 launch (one column or gate) [sync]: out_host[0] = start time, then 4 arrays of U1MPS_MAXSWEEP
+ * entries: end time of each Jacobi sweep (GPU globaltimer, ns), pair items that rotated, inner EVD sweeps run, sectors
+ * still active.  cap (entries of out_host) must be >= 4 * U1MPS_MAXSWEEP + 1. */
+#define U1MPS_MAXSWEEP 30
+int u1mps_svd_trace(u1mps_t* h, long long* out_host, int cap);
+
 /* Number of kernels this handle has launched since create (for bench.py's gpu_launches). */
 int u1mps_launch_count(u1mps_t* h, long long* out_host);
 

@@ -22,7 +22,7 @@ EXPORTS = [
     "u1mps_bond_dims", "u1mps_last_stats", "u1mps_export_bond", "u1mps_export_site", "u1mps_import_bond",
     "u1mps_import_site", "u1mps_set_log_norm", "u1mps_staged_info", "u1mps_export_staged_theta",
     "u1mps_export_staged_svd", "u1mps_launch_count", "u1mps_profile_enable", "u1mps_profile_read",
-    "u1mps_stage_name",
+    "u1mps_stage_name", "u1mps_svd_trace",
 ]
 NSTAGE = 8
 
@@ -82,6 +82,7 @@ def load_library() -> C.CDLL:
     lib.u1mps_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
     lib.u1mps_profile_enable.argtypes = [vp, C.c_int]
     lib.u1mps_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+    lib.u1mps_svd_trace.argtypes = [vp, C.POINTER(C.c_longlong), C.c_int]
     lib.u1mps_stage_name.restype = C.c_char_p
     lib.u1mps_stage_name.argtypes = [C.c_int]
     for name in EXPORTS:
@@ -239,6 +240,16 @@ class U1MPS:
         n = np.zeros(NSTAGE, np.int64)
         self._ck(self.lib.u1mps_profile_read(self.h, _ptr(ms, C.POINTER(C.c_double)), _ptr(n, C.POINTER(C.c_longlong))))
         return {self.lib.u1mps_stage_name(s).decode(): (float(ms[s]), int(n[s])) for s in range(NSTAGE)}
+
+    def svd_trace(self) -> Dict[str, np.ndarray]:
+        """Per-sweep trace of the last a3 launch: ms per sweep, rotated pair items, inner EVD sweeps, active sectors."""
+        ms_ = 30
+        raw = np.zeros(4 * ms_ + 1, np.int64)
+        self._ck(self.lib.u1mps_svd_trace(self.h, _ptr(raw, C.POINTER(C.c_longlong)), len(raw)))
+        t = np.concatenate([[raw[0]], raw[1:1 + ms_]])
+        n = int(np.count_nonzero(raw[1:1 + ms_]))
+        return {"sweep_ms": np.diff(t[:n + 1]) * 1e-6, "rotated_items": raw[1 + ms_:1 + ms_ + n],
+                "inner_sweeps": raw[1 + 2 * ms_:1 + 2 * ms_ + n], "active_sectors": raw[1 + 3 * ms_:1 + 3 * ms_ + n]}
 
     def launch_count(self) -> int:
         v = C.c_longlong()

@@ -49,6 +49,7 @@ Sizes compute_sizes(int M, int d, int N, int chi) {
   add((E + 1) * 8); add((E + 1) * 4);                            // goff svoff
   add((E * d * d + 1) * 4); add((2 * E + 1) * 4);                // t2pref t5pref
   add(8 * 4); add(E * U1_MAXSWEEP * 4); add((size_t)2 * z.Gmax * 8);  // cnt flags gate_w
+  add((4 * U1_MAXSWEEP + 1) * 8);                                // trace
   for (int i = 0; i < 2; ++i) add((size_t)z.itemcap * 4);        // item lists
   add((size_t)z.poolcap * 4); add((size_t)z.poolcap * 8); add((size_t)z.poolcap * 8);  // perm sv svs
   b = (b + 255) & ~(size_t)255;
@@ -210,6 +211,7 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
   P.goff = A.take<long long>(E + 1); P.svoff = A.take<int>(E + 1);
   P.t2pref = A.take<int>(E * d * d + 1); P.t5pref = A.take<int>(2 * E + 1);
   P.cnt = A.take<int>(8); P.flags = A.take<int>(E * U1_MAXSWEEP); P.gate_w = A.take<double>((size_t)2 * z.Gmax);
+  P.trace = A.take<long long>(4 * U1_MAXSWEEP + 1);
   P.pitem_e = A.take<int>(z.itemcap); P.pitem_k = A.take<int>(z.itemcap);
   P.perm = A.take<int>(z.poolcap); P.sv = A.take<double>(z.poolcap); P.svs = A.take<double>(z.poolcap);
   P.poolcap = z.poolcap; P.itemcap = z.itemcap;
@@ -644,6 +646,13 @@ const char* u1mps_stage_name(int stage) {
   static const char* names[U1MPS_NSTAGE] = {"a1_plan", "a2_contract", "a2_identity", "a3_svd", "a3_sigma_sort",
                                             "a4_select", "a5_scatter", "a6_readout"};
   return (stage >= 0 && stage < U1MPS_NSTAGE) ? names[stage] : "";
+}
+
+int u1mps_svd_trace(u1mps_t* h, long long* out, int cap) {
+  if (!h || !out || cap < 4 * U1_MAXSWEEP + 1) return U1MPS_EINVAL;
+  CK(cudaMemcpyAsync(out, h->P.trace, (4 * U1_MAXSWEEP + 1) * 8, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return U1MPS_OK;
 }
 
 int u1mps_launch_count(u1mps_t* h, long long* out) {

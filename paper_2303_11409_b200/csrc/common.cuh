@@ -11,7 +11,7 @@ typedef double2 cplx;  // complex128, interleaved (x = re, y = im), 16-byte alig
 #define U1_PANEL 16        // (item-list sizing unit)
 #define U1_PB 16           // columns per Jacobi panel: a pair item orthogonalises 2*U1_PB = 32 columns
 #define U1_ERR_WORKSPACE 1 // device error flag: plan does not fit the workspace
-#define U1_SVD_THREADS 256 // 8 warps: DMMA tiles of the Gram / update GEMMs, 16 x 16 two-by-two units of the inner EVD
+#define U1_SVD_THREADS 128 // 4 warps per pair item (4 CTAs per SM): DMMA tile rows / columns of the Gram / update GEMMs
 #define U1MPS_SORT_MAX 4096 // largest sector the in-smem bitonic sort takes (= U1MPS_CHI_MAX)
 
 // Persistent MPS state (all device pointers into the caller's arena).
@@ -44,6 +44,7 @@ struct Plan {
   int* tmpa;         // [G*NC+1] scratch: pair-item offset per entry
   int* cnt;          // [8] 0: #blk, 1: #pair items, 3: max panels (even), 4: a2 tiles, 5: a5 tiles, 6: a3 work-queue ticket, 7: a4 CTA counter
   int* flags;        // [G*NC*U1_MAXSWEEP] per entry, per sweep: 1 if any rotation happened
+  long long* trace;  // [4*U1_MAXSWEEP] a3 trace of the last launch: per sweep end time (globaltimer ns), rotated items, inner sweeps, active sectors
   int* keep;         // [G*NC] kept singular values per entry (a4)
   int* perm;         // [pool] sorted position -> column index
   double* sv;        // [pool] unsorted column norms

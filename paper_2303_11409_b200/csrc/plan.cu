@@ -109,6 +109,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
   }
   atomicMax(&shmax, mymax);
   for (int i = t; i < E * U1_MAXSWEEP; i += PLAN_THREADS) P.flags[i] = 0;
+  for (int i = t; i < 4 * U1_MAXSWEEP + 1; i += PLAN_THREADS) P.trace[i] = 0;
   __syncthreads();
   if (t == 0) P.cnt[3] = shmax;
 }

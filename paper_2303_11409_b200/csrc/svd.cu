@@ -7,10 +7,10 @@
 //
 // Blocking.  Columns are grouped in panels of U1_PB = 16.  A work item is a panel pair P = [Pa Pb]
 // (32 columns):
-//   1. Gram   H = P^H P over the m rows of G           (FP64 DMMA.8x8x4 tiles, chunks of 64 rows staged
+//   1. Gram   H = P^H P over the m rows of G           (FP64 DMMA.8x8x4 tiles, chunks of 32 rows staged
 //                                                        in shared memory by a 3-stage cp.async ring)
 //   2. EVD    H = Q diag Q^H by two-sided Jacobi in shared memory (parallel round-robin ordering, 16
-//             rotations per round, 16 x 16 two-by-two units, one per thread; rotations sort the pair by
+//             rotations per round on two-by-two units, in place; rotations sort the pair by
 //             norm, de Rijk style, which is what makes graded spectra converge)
 //   3. update [Pa Pb] <- [Pa Pb] Q over all m + n rows  (DMMA again, Q held in registers as B fragments)
 // A persistent cooperative grid walks the round-robin tournament of panel pairs of every sector in
@@ -22,15 +22,16 @@
 namespace cg = cooperative_groups;
 
 #define SV_W 32                      // columns of a pair item
-#define SV_R 64                      // rows per staged chunk
-#define SV_LDG 68                    // shared-memory leading dimension (complex elements) in the Gram phase: 4 mod 8
-#define SV_LDU 66                    // ... in the update phase: 2 mod 8 (both: conflict-free LDS.128 fragment loads)
+#define SV_R 32                      // rows per staged chunk
+#define SV_LDG 36                    // shared-memory leading dimension (complex elements) in the Gram phase: 4 mod 8
+#define SV_LDU 34                    // ... in the update phase: 2 mod 8 (both: conflict-free LDS.128 fragment loads)
 #define SV_STAGE (SV_W * SV_LDG)     // complex elements per stage
 #define SV_NSTAGE 3
-#define SV_HLD 33                    // leading dimension of the 32 x 32 Gram / eigenvector matrices
+#define SV_HLD 33                    // leading dimension of the 32 x 32 Gram matrix (row-major)
+#define SV_QLD 36                    // leading dimension of the transposed eigenvector matrix Qt (4 mod 8: B fragments)
 #define SV_INNER_MAX 3               // inner EVD sweeps per item (the outer iteration finishes the job)
 #define SV_QUAD 1e-14                // stop the inner EVD after a sweep whose largest relative off-diagonal^2 was below this
-#define SV_SMEM_BYTES (SV_NSTAGE * SV_STAGE * 16)
+#define SV_SMEM_BYTES (SV_NSTAGE * SV_STAGE * 16)   // 55,296 B: four CTAs of 128 threads per SM
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -74,14 +75,14 @@ struct Item {
   double tol2;
 };
 
-// Stage rows [row0, row0 + 64) x the 32 columns of the item into shared memory (column-major, leading dimension ld);
+// Stage rows [row0, row0 + SV_R) x the 32 columns of the item into shared memory (column-major, leading dimension ld);
 // rows >= rowlim and absent columns are zero-filled.
 __device__ __forceinline__ void load_chunk(cplx* st, int ld, const Item& I, int row0, int rowlim) {
   const int r = threadIdx.x & (SV_R - 1);
   const bool rok = row0 + r < rowlim;
 #pragma unroll
   for (int it = 0; it < SV_W * SV_R / U1_SVD_THREADS; ++it) {
-    const int j = (threadIdx.x >> 6) + it * (U1_SVD_THREADS / SV_R);
+    const int j = threadIdx.x / SV_R + it * (U1_SVD_THREADS / SV_R);
     const bool ok = rok && (j < U1_PB ? j < I.na : j - U1_PB < I.nb);
     const long long gcol = j < U1_PB ? I.ca + j : I.cb + j - U1_PB;
     const cplx* src = ok ? I.W + gcol * I.mt + row0 + r : I.W;
@@ -89,12 +90,13 @@ __device__ __forceinline__ void load_chunk(cplx* st, int ld, const Item& I, int 
   }
 }
 
-// ---- phase 1: H = P^H P over rows [0, m).  Warp w owns tile row w/2 and tile columns 2(w%2), 2(w%2)+1 of the 4 x 4 tiles.
+// ---- phase 1: H = P^H P over rows [0, m).  Warp w owns tile row w of the 4 x 4 tiles (8 x 8 each).
 __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int ti = warp >> 1, tj = (warp & 1) * 2;
+  const int lane = threadIdx.x & 31, ti = threadIdx.x >> 5;
   const int lr = lane >> 2, lk = lane & 3;
-  double cre[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, cim[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+  double cre[4][2], cim[4][2];
+#pragma unroll
+  for (int u = 0; u < 4; ++u) { cre[u][0] = cre[u][1] = 0.0; cim[u][0] = cim[u][1] = 0.0; }
   const int nch = (I.m + SV_R - 1) / SV_R;
   load_chunk(stages, SV_LDG, I, 0, I.m);
   cp_async_commit();
@@ -109,26 +111,27 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
     const int rows = min(SV_R, I.m - c * SV_R);
     const int nk = (rows + 3) >> 2;
     const cplx* pa = st + (8 * ti + lr) * SV_LDG + lk;
-    const cplx* pb0 = st + (8 * tj + lr) * SV_LDG + lk;
-    const cplx* pb1 = pb0 + 8 * SV_LDG;
-#pragma unroll 4
+    const cplx* pb = st + lr * SV_LDG + lk;
+#pragma unroll 2
     for (int ks = 0; ks < nk; ++ks) {
-      const cplx a = pa[4 * ks], b0 = pb0[4 * ks], b1 = pb1[4 * ks];
+      const cplx a = pa[4 * ks];
       const double nai = -a.y;
-      // conj(a) * b : re = ar br + ai bi ; im = ar bi - ai br
-      dmma(cre[0][0], cre[0][1], a.x, b0.x); dmma(cre[0][0], cre[0][1], a.y, b0.y);
-      dmma(cim[0][0], cim[0][1], a.x, b0.y); dmma(cim[0][0], cim[0][1], nai, b0.x);
-      dmma(cre[1][0], cre[1][1], a.x, b1.x); dmma(cre[1][0], cre[1][1], a.y, b1.y);
-      dmma(cim[1][0], cim[1][1], a.x, b1.y); dmma(cim[1][0], cim[1][1], nai, b1.x);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const cplx b = pb[u * 8 * SV_LDG + 4 * ks];
+        // conj(a) * b : re = ar br + ai bi ; im = ar bi - ai br
+        dmma(cre[u][0], cre[u][1], a.x, b.x); dmma(cre[u][0], cre[u][1], a.y, b.y);
+        dmma(cim[u][0], cim[u][1], a.x, b.y); dmma(cim[u][0], cim[u][1], nai, b.x);
+      }
     }
   }
   cp_async_wait<0>();
   __syncthreads();  // every warp is done with the stages: Hs (aliased onto stages 1..2) may be written
 #pragma unroll
-  for (int u = 0; u < 2; ++u)
+  for (int u = 0; u < 4; ++u)
 #pragma unroll
     for (int t = 0; t < 2; ++t)
-      Hs[(8 * ti + lr) * SV_HLD + 8 * (tj + u) + 2 * lk + t] = make_double2(cre[u][t], cim[u][t]);
+      Hs[(8 * ti + lr) * SV_HLD + 8 * u + 2 * lk + t] = make_double2(cre[u][t], cim[u][t]);
   __syncthreads();
   // exact Hermitian symmetry from the upper triangle (the quick test and the rotations read p < q only)
   for (int idx = threadIdx.x; idx < SV_W * SV_W; idx += U1_SVD_THREADS) {
@@ -139,25 +142,46 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
   __syncthreads();
 }
 
-// ---- phase 2: two-sided Jacobi EVD of the Hermitian H (2*hp x 2*hp, hp = 16 or 8 pairs per round), Q accumulates the
-// rotations.  H and Q are double-buffered (Hs/Qs: [2][32*33]); returns the index of the buffer holding the result.
-// Rotation of the pivot (p, q), p < q (same formulas as a scalar one-sided rotation of columns p, q, whose Gram
-// entries are a = h_pp, b = h_qq, g = h_pq):  zeta = (b - a) / (2|g|), t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)),
-// cs = 1/sqrt(1 + t^2), s = cs t g/|g|,  R = [[cs, s], [-conj(s), cs]]; if the new norms a - t|g| < b + t|g| the two
-// columns of R are swapped so that the larger norm ends up in the lower column.
-__device__ __forceinline__ int evd_phase(cplx* Hs, cplx* Qs, cplx (*Rm)[4], int* sp, int* sq, int hp, double tol2) {
+// pivot k of round t of the round-robin tournament over np2 players (not ordered: consecutive k give consecutive
+// indices, which keeps the shared-memory accesses of a quarter warp in distinct banks)
+__device__ __forceinline__ void pivot(int t, int k, int np2, int* p, int* q) {
+  const int m = np2 - 1;
+  if (k == 0) { *p = t; *q = m; return; }
+  int a = t + k, b = t - k + m;
+  if (a >= m) a -= m;
+  if (b >= m) b -= m;
+  *p = a; *q = b;
+}
+__device__ __forceinline__ double rsqrt_approx(double x) { double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
+__device__ __forceinline__ double rcp_approx(double x) { double y; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
+
+// ---- phase 2: two-sided Jacobi EVD of the Hermitian H (2*hp x 2*hp, hp = 16 or 8 pivots per round), Qt (stored
+// transposed) accumulates the rotations; both in place in shared memory: in a round the 2 x 2 unit (rows of pivot ki,
+// columns of pivot kj) is read and written by one thread only.  H stays exactly Hermitian: only units ki <= kj are
+// computed, each written together with its mirror image.
+// Rotation of the pivot (p, q) (a scalar one-sided rotation of columns p, q, whose Gram entries are a = h_pp, b = h_qq,
+// g = h_pq):  zeta = (b - a) / (2|g|), t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)), tau = t g/|g|,
+// R = [[1, tau], [-conj(tau), 1]] / sqrt(1 + |tau|^2).  tau comes from the ~20-bit MUFU reciprocal / rsqrt (it only has
+// to shrink the off-diagonal entry; the iteration is self-correcting), the normalisation is done in full precision so
+// that R is unitary to rounding whatever tau is.  The columns of R are swapped where needed so that the larger norm
+// ends up in the column with the lower index (de Rijk).
+__device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int* srot, int hp, double tol2, int* inner) {
   const int tid = threadIdx.x;
   const int np2 = 2 * hp;
-  for (int idx = tid; idx < SV_W * SV_W; idx += U1_SVD_THREADS) {  // both buffers: a round rewrites only the 2hp x 2hp corner
-    const int r = idx >> 5, c = idx & 31;
-    const cplx one = make_double2(r == c ? 1.0 : 0.0, 0.0);
-    Qs[r * SV_HLD + c] = one;
-    Qs[SV_W * SV_HLD + r * SV_HLD + c] = one;
-    Hs[SV_W * SV_HLD + r * SV_HLD + c] = Hs[r * SV_HLD + c];
+  for (int idx = tid; idx < SV_W * SV_QLD; idx += U1_SVD_THREADS) {
+    const int c = idx / SV_QLD, r = idx - c * SV_QLD;
+    Qt[idx] = make_double2(r == c ? 1.0 : 0.0, 0.0);
   }
-  int cur = 0;
-  const int ki = tid / hp, kj = tid % hp;
-  const bool worker = tid < hp * hp;
+  // H units of this thread: entries tid and tid + 128 of the row-major list of the upper triangle ki <= kj
+  const int nunit = hp * (hp + 1) / 2;
+  int uki[2], ukj[2];
+#pragma unroll
+  for (int x = 0; x < 2; ++x) {
+    int u = tid + x * U1_SVD_THREADS, ki = 0;
+    if (u >= nunit) { uki[x] = -1; ukj[x] = 0; continue; }
+    while (u >= hp - ki) { u -= hp - ki; ++ki; }
+    uki[x] = ki; ukj[x] = ki + u;
+  }
   __syncthreads();
   for (int sw = 0; sw < SV_INNER_MAX; ++sw) {
     double mymax = 0.0;
@@ -166,22 +190,28 @@ __device__ __forceinline__ int evd_phase(cplx* Hs, cplx* Qs, cplx (*Rm)[4], int*
       int rot = 0;
       if (tid < hp) {
         int p, q;
-        rr_pair(t, tid, np2, &p, &q);
-        const cplx* H = Hs + cur * (SV_W * SV_HLD);
+        pivot(t, tid, np2, &p, &q);
         const double a = H[p * SV_HLD + p].x, b = H[q * SV_HLD + q].x;
         const cplx g = H[p * SV_HLD + q];
         const double g2 = g.x * g.x + g.y * g.y, ab = a * b;
         cplx r00 = make_double2(1.0, 0.0), r01 = make_double2(0.0, 0.0), r10 = r01, r11 = r00;
-        if (ab > 0.0 && g2 > tol2 * ab) {
+        if (ab > 0.0 && g2 > tol2 * ab && g2 > 1e-290) {
           rot = 1;
-          mymax = fmax(mymax, g2 / ab);
-          const double ag = sqrt(g2);
-          const double zeta = (b - a) / (2.0 * ag);
-          const double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-          const double cs = rsqrt(1.0 + tt * tt);
-          const double sn = cs * tt;
-          const double sr = sn * g.x / ag, si = sn * g.y / ag;
-          if ((a - tt * ag) < (b + tt * ag)) {  // swapped columns
+          mymax = fmax(mymax, g2 * rcp_approx(ab));
+          const double iag = rsqrt_approx(g2);                 // ~ 1/|g|
+          const double zeta = 0.5 * (b - a) * iag;
+          const double z1 = fma(zeta, zeta, 1.0);
+          const double tt = copysign(rcp_approx(fabs(zeta) + z1 * rsqrt_approx(z1)), zeta);
+          const double ti = tt * iag;
+          const double tx = ti * g.x, ty = ti * g.y;           // tau
+          const double n2 = fma(tx, tx, fma(ty, ty, 1.0));
+          double cs = rsqrt_approx(n2);                        // two Newton steps: full precision
+          cs = fma(0.5 * cs, fma(-n2 * cs, cs, 1.0), cs);
+          cs = fma(0.5 * cs, fma(-n2 * cs, cs, 1.0), cs);
+          const double sr = cs * tx, si = cs * ty;
+          const double dn = tt * g2 * iag;                     // norms after the rotation: a - dn (column p), b + dn (column q)
+          const bool swp = (p < q) ? (a - dn < b + dn) : (b + dn < a - dn);
+          if (swp) {
             r00 = make_double2(sr, si); r01 = make_double2(cs, 0.0);
             r10 = make_double2(cs, 0.0); r11 = make_double2(-sr, si);
           } else {
@@ -190,54 +220,75 @@ __device__ __forceinline__ int evd_phase(cplx* Hs, cplx* Qs, cplx (*Rm)[4], int*
           }
         }
         Rm[tid][0] = r00; Rm[tid][1] = r01; Rm[tid][2] = r10; Rm[tid][3] = r11;
-        sp[tid] = p; sq[tid] = q;
+        srot[tid] = rot;
+      }
+      // pivots of this thread's units (integer work, overlaps the rotation parameters of warp 0)
+      int pi[2], qi[2], pj[2], qj[2];
+#pragma unroll
+      for (int x = 0; x < 2; ++x) {
+        pivot(t, max(uki[x], 0), np2, &pi[x], &qi[x]);
+        pivot(t, ukj[x], np2, &pj[x], &qj[x]);
       }
       const int any = __syncthreads_or(rot);
-      if (!any) continue;  // nobody rotated: buffers stay as they are (uniform branch)
+      if (!any) continue;  // nobody rotated in this round (uniform branch)
       sweep_any = 1;
-      if (worker) {
-        const cplx* H = Hs + cur * (SV_W * SV_HLD);
-        cplx* Hn = Hs + (cur ^ 1) * (SV_W * SV_HLD);
-        const cplx* Q = Qs + cur * (SV_W * SV_HLD);
-        cplx* Qn = Qs + (cur ^ 1) * (SV_W * SV_HLD);
-        const int pi = sp[ki], qi = sq[ki], pj = sp[kj], qj = sq[kj];
+#pragma unroll
+      for (int x = 0; x < 2; ++x) {
+        const int ki = uki[x], kj = ukj[x];
+        if (ki < 0) continue;
         const cplx j00 = Rm[kj][0], j01 = Rm[kj][1], j10 = Rm[kj][2], j11 = Rm[kj][3];
         const cplx i00 = Rm[ki][0], i01 = Rm[ki][1], i10 = Rm[ki][2], i11 = Rm[ki][3];
-        const cplx b00 = H[pi * SV_HLD + pj], b01 = H[pi * SV_HLD + qj], b10 = H[qi * SV_HLD + pj], b11 = H[qi * SV_HLD + qj];
+        const cplx b00 = H[pi[x] * SV_HLD + pj[x]], b01 = H[pi[x] * SV_HLD + qj[x]];
+        const cplx b10 = H[qi[x] * SV_HLD + pj[x]], b11 = H[qi[x] * SV_HLD + qj[x]];
+        if (!(srot[ki] | srot[kj])) continue;  // both pivots idle
         // T = B Rj ; B' = Ri^H T
         const cplx t00 = cadd(cmul(b00, j00), cmul(b01, j10)), t01 = cadd(cmul(b00, j01), cmul(b01, j11));
         const cplx t10 = cadd(cmul(b10, j00), cmul(b11, j10)), t11 = cadd(cmul(b10, j01), cmul(b11, j11));
-        Hn[pi * SV_HLD + pj] = cadd(cmulc(i00, t00), cmulc(i10, t10));
-        Hn[pi * SV_HLD + qj] = cadd(cmulc(i00, t01), cmulc(i10, t11));
-        Hn[qi * SV_HLD + pj] = cadd(cmulc(i01, t00), cmulc(i11, t10));
-        Hn[qi * SV_HLD + qj] = cadd(cmulc(i01, t01), cmulc(i11, t11));
-        // Q rows 2ki, 2ki+1, columns (pj, qj):  Q' = Q Rj
-        const int r0 = 2 * ki, r1 = r0 + 1;
-        const cplx q00 = Q[r0 * SV_HLD + pj], q01 = Q[r0 * SV_HLD + qj], q10 = Q[r1 * SV_HLD + pj], q11 = Q[r1 * SV_HLD + qj];
-        Qn[r0 * SV_HLD + pj] = cadd(cmul(q00, j00), cmul(q01, j10));
-        Qn[r0 * SV_HLD + qj] = cadd(cmul(q00, j01), cmul(q01, j11));
-        Qn[r1 * SV_HLD + pj] = cadd(cmul(q10, j00), cmul(q11, j10));
-        Qn[r1 * SV_HLD + qj] = cadd(cmul(q10, j01), cmul(q11, j11));
+        cplx n00 = cadd(cmulc(i00, t00), cmulc(i10, t10)), n01 = cadd(cmulc(i00, t01), cmulc(i10, t11));
+        cplx n10 = cadd(cmulc(i01, t00), cmulc(i11, t10)), n11 = cadd(cmulc(i01, t01), cmulc(i11, t11));
+        if (ki == kj) {  // the pivot block itself: diagonal by construction
+          n00.y = 0.0; n11.y = 0.0;
+          n01 = make_double2(0.0, 0.0); n10 = n01;
+          H[pi[x] * SV_HLD + pi[x]] = n00; H[pi[x] * SV_HLD + qi[x]] = n01; H[qi[x] * SV_HLD + pi[x]] = n10; H[qi[x] * SV_HLD + qi[x]] = n11;
+        } else {
+          H[pi[x] * SV_HLD + pj[x]] = n00; H[pi[x] * SV_HLD + qj[x]] = n01; H[qi[x] * SV_HLD + pj[x]] = n10; H[qi[x] * SV_HLD + qj[x]] = n11;
+          H[pj[x] * SV_HLD + pi[x]] = make_double2(n00.x, -n00.y); H[qj[x] * SV_HLD + pi[x]] = make_double2(n01.x, -n01.y);
+          H[pj[x] * SV_HLD + qi[x]] = make_double2(n10.x, -n10.y); H[qj[x] * SV_HLD + qi[x]] = make_double2(n11.x, -n11.y);
+        }
       }
-      cur ^= 1;
+      // Q rows (rp, rp + hp), columns (pj, qj):  Q' = Q Rj ; Qt is column-major, consecutive threads take consecutive rows
+      for (int u = tid; u < hp * hp; u += U1_SVD_THREADS) {
+        const int kj = u / hp, rp = u - kj * hp;
+        int pc, qc;
+        pivot(t, kj, np2, &pc, &qc);
+        const cplx j00 = Rm[kj][0], j01 = Rm[kj][1], j10 = Rm[kj][2], j11 = Rm[kj][3];
+        if (!srot[kj]) continue;
+        cplx* cp = Qt + pc * SV_QLD + rp;
+        cplx* cq = Qt + qc * SV_QLD + rp;
+        const cplx q00 = cp[0], q01 = cq[0], q10 = cp[hp], q11 = cq[hp];
+        cp[0] = cadd(cmul(q00, j00), cmul(q01, j10));
+        cq[0] = cadd(cmul(q00, j01), cmul(q01, j11));
+        cp[hp] = cadd(cmul(q10, j00), cmul(q11, j10));
+        cq[hp] = cadd(cmul(q10, j01), cmul(q11, j11));
+      }
       __syncthreads();
     }
     if (!sweep_any) break;
+    ++*inner;
     if (!__syncthreads_or(mymax > SV_QUAD)) break;
   }
-  return cur;
 }
 
-// ---- phase 3: [Pa Pb] <- [Pa Pb] Q over all mt rows.  Warp w owns tile column w%4 (8 columns) and the row tiles
-// (w/4), (w/4)+2, ... of each 64-row chunk; its 32 x 8 slice of Q lives in registers as 8 B fragments.
-__device__ __forceinline__ void update_phase(cplx* stages, const cplx* Q, const Item& I) {
+// ---- phase 3: [Pa Pb] <- [Pa Pb] Q over all mt rows.  Warp w owns tile column w (8 columns) and all row tiles
+// of each 32-row chunk; its 32 x 8 slice of Q lives in registers as 8 B fragments.
+__device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const Item& I) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int tj = warp & 3, rh = warp >> 2;
+  const int tj = warp;
   const int lr = lane >> 2, lk = lane & 3;
   double bre[8], bim[8];
 #pragma unroll
   for (int ks = 0; ks < 8; ++ks) {
-    const cplx v = Q[(4 * ks + lk) * SV_HLD + 8 * tj + lr];
+    const cplx v = Qt[(8 * tj + lr) * SV_QLD + 4 * ks + lk];   // Q[k][j], k = 4 ks + lk, j = 8 tj + lr
     bre[ks] = v.x; bim[ks] = v.y;
   }
   __syncthreads();  // Q (aliased onto stages 1..2) is in registers everywhere: the ring may be refilled
@@ -263,7 +314,7 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Q, const 
     const int row0 = c * SV_R;
     const int rows = min(SV_R, I.mt - row0);
 #pragma unroll
-    for (int rt = rh; rt < SV_R / 8; rt += 2) {
+    for (int rt = 0; rt < SV_R / 8; ++rt) {
       if (8 * rt >= rows) break;
       double cre[2] = {0.0, 0.0}, cim[2] = {0.0, 0.0};
       const cplx* pa = st + lk * SV_LDU + 8 * rt + lr;
@@ -286,13 +337,13 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Q, const 
   __syncthreads();
 }
 
-__global__ void __launch_bounds__(U1_SVD_THREADS, 2) svd_kernel(DevState S, Plan P) {
+__global__ void __launch_bounds__(U1_SVD_THREADS, 4) svd_kernel(DevState S, Plan P) {
   extern __shared__ __align__(16) unsigned char smraw[];
   cplx* stages = reinterpret_cast<cplx*>(smraw);
-  cplx* Hs = stages + SV_STAGE;                    // [2][32*33], aliased onto stages 1..2 (idle during the EVD)
-  cplx* Qs = Hs + 2 * SV_W * SV_HLD;               // [2][32*33]
+  cplx* Hs = stages + SV_STAGE;                    // [32*33], aliased onto stages 1..2 (idle during the EVD)
+  cplx* Qs = Hs + SV_W * SV_HLD;                   // [32*36], transposed
   __shared__ cplx Rm[U1_PB][4];
-  __shared__ int sp[U1_PB], sq[U1_PB];
+  __shared__ int srot[U1_PB];
   __shared__ unsigned s_ticket;
   cg::grid_group grid = cg::this_grid();
   const int nblk = P.cnt[0], npair = P.cnt[1], maxP = P.cnt[3];
@@ -301,7 +352,9 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, 2) svd_kernel(DevState S, Plan
   unsigned base = 0;
   unsigned* ticket = reinterpret_cast<unsigned*>(P.cnt + 6);
   int sweep = 0;
+  if (blockIdx.x == 0 && tid == 0) { long long t0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0)); P.trace[0] = t0; }
   for (; sweep < U1_MAXSWEEP && nblk > 0; ++sweep) {
+    int n_rot = 0, n_inner = 0;
     for (int t = 0; t < rounds; ++t) {
       for (;;) {
         __syncthreads();
@@ -341,16 +394,30 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, 2) svd_kernel(DevState S, Plan
         }
         if (!__syncthreads_or(todo)) continue;
         if (tid == 0) P.flags[e * U1_MAXSWEEP + sweep] = 1;
-        const int cur = evd_phase(Hs, Qs, Rm, sp, sq, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2);
-        update_phase(stages, Qs + cur * (SV_W * SV_HLD), I);
+        int inner = 0;
+        evd_phase(Hs, Qs, Rm, srot, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner);
+        update_phase(stages, Qs, I);
+        n_rot += 1; n_inner += inner;
       }
       base += (unsigned)npair + gridDim.x;
       grid.sync();
     }
     // ---- convergence: stop when no sector rotated in this sweep
     int any = 0;
-    for (int bi = tid; bi < nblk; bi += U1_SVD_THREADS) any |= __ldcg(&P.flags[P.blk[bi] * U1_MAXSWEEP + sweep]);
-    if (!__syncthreads_or(any)) { ++sweep; break; }
+    for (int bi = tid; bi < nblk; bi += U1_SVD_THREADS) any += __ldcg(&P.flags[P.blk[bi] * U1_MAXSWEEP + sweep]);
+    const int nact = __syncthreads_count(any);  // (threads that saw an active sector; exact count below)
+    if (tid == 0) {  // trace of this launch (u1mps_svd_trace)
+      if (n_rot) { atomicAdd((unsigned long long*)&P.trace[1 + U1_MAXSWEEP + sweep], (unsigned long long)n_rot);
+                   atomicAdd((unsigned long long*)&P.trace[1 + 2 * U1_MAXSWEEP + sweep], (unsigned long long)n_inner); }
+      if (blockIdx.x == 0) {
+        long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+        P.trace[1 + sweep] = t1;
+        int act = 0;
+        for (int bi = 0; bi < nblk; ++bi) act += __ldcg(&P.flags[P.blk[bi] * U1_MAXSWEEP + sweep]);
+        P.trace[1 + 3 * U1_MAXSWEEP + sweep] = act;
+      }
+    }
+    if (nact == 0) { ++sweep; break; }
   }
   if (blockIdx.x == 0 && tid == 0) {
     atomicMax(&S.err[1], sweep);
