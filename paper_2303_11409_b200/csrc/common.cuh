@@ -11,7 +11,7 @@ typedef double2 cplx;  // complex128, interleaved (x = re, y = im), 16-byte alig
 #define U1_PANEL 16        // (item-list sizing unit)
 #define U1_PB 16           // columns per Jacobi panel: a pair item orthogonalises 2*U1_PB = 32 columns
 #define U1_ERR_WORKSPACE 1 // device error flag: plan does not fit the workspace
-#define U1_SVD_THREADS 128 // 4 warps per pair item (4 CTAs per SM): DMMA tile rows / columns of the Gram / update GEMMs
+#define U1_SVD_THREADS 128 // 4 warps per pair item, 6 CTAs per SM
 #define U1MPS_SORT_MAX 4096 // largest sector the in-smem bitonic sort takes (= U1MPS_CHI_MAX)
 
 // Persistent MPS state (all device pointers into the caller's arena).

@@ -8,7 +8,7 @@
 // Blocking.  Columns are grouped in panels of U1_PB = 16.  A work item is a panel pair P = [Pa Pb]
 // (32 columns):
 //   1. Gram   H = P^H P over the m rows of G           (FP64 DMMA.8x8x4 tiles, chunks of 32 rows staged
-//                                                        in shared memory by a 3-stage cp.async ring)
+//                                                        in shared memory by a 2-stage cp.async ring)
 //   2. EVD    H = Q diag Q^H by two-sided Jacobi in shared memory (parallel round-robin ordering, 16
 //             rotations per round on two-by-two units, in place; rotations sort the pair by
 //             norm, de Rijk style, which is what makes graded spectra converge)
@@ -18,6 +18,7 @@
 // decided on the device per sector (a sweep in which no item had an off-diagonal Gram entry above
 // tol * sqrt(h_pp h_qq)), no host round trip.
 #include <cooperative_groups.h>
+#include <cstdlib>
 #include "common.cuh"
 namespace cg = cooperative_groups;
 
@@ -26,12 +27,16 @@ namespace cg = cooperative_groups;
 #define SV_LDG 36                    // shared-memory leading dimension (complex elements) in the Gram phase: 4 mod 8
 #define SV_LDU 34                    // ... in the update phase: 2 mod 8 (both: conflict-free LDS.128 fragment loads)
 #define SV_STAGE (SV_W * SV_LDG)     // complex elements per stage
-#define SV_NSTAGE 3
+#define SV_NSTAGE 2
 #define SV_HLD 33                    // leading dimension of the 32 x 32 Gram matrix (row-major)
 #define SV_QLD 36                    // leading dimension of the transposed eigenvector matrix Qt (4 mod 8: B fragments)
 #define SV_INNER_MAX 3               // inner EVD sweeps per item (the outer iteration finishes the job)
 #define SV_QUAD 1e-14                // stop the inner EVD after a sweep whose largest relative off-diagonal^2 was below this
-#define SV_SMEM_BYTES (SV_NSTAGE * SV_STAGE * 16)   // 55,296 B: four CTAs of 128 threads per SM
+#define SV_GROUP 128                 // threads per pair item; a CTA runs U1_SVD_THREADS / SV_GROUP = 4 items in lock-stepped phases
+#define SV_NGROUP (U1_SVD_THREADS / SV_GROUP)
+#define SV_CTAS 6                    // resident CTAs per SM the kernel is compiled for (registers <= 85)
+#define SV_GROUP_BYTES (SV_NSTAGE * SV_STAGE * 16)   // 55,296 B per group
+#define SV_SMEM_BYTES (SV_NGROUP * SV_GROUP_BYTES)
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -53,11 +58,33 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
+// Named barriers of a 128-thread group (ids 1..4; 0 is __syncthreads) and its block-wide OR.
+__device__ __forceinline__ void gsync(int g) { asm volatile("bar.sync %0, 128;\n" ::"r"(g + 1) : "memory"); }
+__device__ __forceinline__ int gsync_or(int g, int pred) {
+  int r;
+  asm volatile("{\n .reg .pred p, q;\n setp.ne.s32 p, %2, 0;\n bar.red.or.pred q, %1, 128, p;\n selp.s32 %0, 1, 0, q;\n}\n"
+               : "=r"(r) : "r"(g + 1), "r"(pred) : "memory");
+  return r;
+}
+
 __device__ __forceinline__ cplx cmul(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ cplx cmulc(cplx a, cplx b) {  // conj(a) * b
   return make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
 }
 __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+// a b + c d  and  conj(a) b + conj(c) d, as fused chains (8 FP64 instructions each)
+__device__ __forceinline__ cplx cdot2(cplx a, cplx b, cplx c, cplx d) {
+#ifdef U1_SLOWCPLX
+  return cadd(cmul(a, b), cmul(c, d));
+#endif
+  return make_double2(fma(a.x, b.x, fma(-a.y, b.y, fma(c.x, d.x, -c.y * d.y))), fma(a.x, b.y, fma(a.y, b.x, fma(c.x, d.y, c.y * d.x))));
+}
+__device__ __forceinline__ cplx cdot2c(cplx a, cplx b, cplx c, cplx d) {
+#ifdef U1_SLOWCPLX
+  return cadd(cmulc(a, b), cmulc(c, d));
+#endif
+  return make_double2(fma(a.x, b.x, fma(a.y, b.y, fma(c.x, d.x, c.y * d.y))), fma(a.x, b.y, fma(-a.y, b.x, fma(c.x, d.y, -c.y * d.x))));
+}
 
 // circle-method round robin over np2 (even) players: slot k of round t -> (a, b), a < b
 __device__ __forceinline__ void rr_pair(int t, int k, int np2, int* a, int* b) {
@@ -77,12 +104,12 @@ struct Item {
 
 // Stage rows [row0, row0 + SV_R) x the 32 columns of the item into shared memory (column-major, leading dimension ld);
 // rows >= rowlim and absent columns are zero-filled.
-__device__ __forceinline__ void load_chunk(cplx* st, int ld, const Item& I, int row0, int rowlim) {
-  const int r = threadIdx.x & (SV_R - 1);
+__device__ __forceinline__ void load_chunk(cplx* st, int ld, const Item& I, int row0, int rowlim, int gtid) {
+  const int r = gtid & (SV_R - 1);
   const bool rok = row0 + r < rowlim;
 #pragma unroll
-  for (int it = 0; it < SV_W * SV_R / U1_SVD_THREADS; ++it) {
-    const int j = threadIdx.x / SV_R + it * (U1_SVD_THREADS / SV_R);
+  for (int it = 0; it < SV_W * SV_R / SV_GROUP; ++it) {
+    const int j = gtid / SV_R + it * (SV_GROUP / SV_R);
     const bool ok = rok && (j < U1_PB ? j < I.na : j - U1_PB < I.nb);
     const long long gcol = j < U1_PB ? I.ca + j : I.cb + j - U1_PB;
     const cplx* src = ok ? I.W + gcol * I.mt + row0 + r : I.W;
@@ -91,21 +118,19 @@ __device__ __forceinline__ void load_chunk(cplx* st, int ld, const Item& I, int 
 }
 
 // ---- phase 1: H = P^H P over rows [0, m).  Warp w owns tile row w of the 4 x 4 tiles (8 x 8 each).
-__device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I) {
-  const int lane = threadIdx.x & 31, ti = threadIdx.x >> 5;
+__device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I, int g, int gtid) {
+  const int lane = gtid & 31, ti = gtid >> 5;
   const int lr = lane >> 2, lk = lane & 3;
   double cre[4][2], cim[4][2];
 #pragma unroll
   for (int u = 0; u < 4; ++u) { cre[u][0] = cre[u][1] = 0.0; cim[u][0] = cim[u][1] = 0.0; }
   const int nch = (I.m + SV_R - 1) / SV_R;
-  load_chunk(stages, SV_LDG, I, 0, I.m);
-  cp_async_commit();
-  if (nch > 1) load_chunk(stages + SV_STAGE, SV_LDG, I, SV_R, I.m);
+  load_chunk(stages, SV_LDG, I, 0, I.m, gtid);
   cp_async_commit();
   for (int c = 0; c < nch; ++c) {
-    cp_async_wait<1>();
-    __syncthreads();
-    if (c + 2 < nch) load_chunk(stages + ((c + 2) % SV_NSTAGE) * SV_STAGE, SV_LDG, I, (c + 2) * SV_R, I.m);
+    cp_async_wait<0>();
+    gsync(g);  // chunk c has landed for everybody, and everybody is done with chunk c - 1: its stage may be refilled
+    if (c + 1 < nch) load_chunk(stages + ((c + 1) % SV_NSTAGE) * SV_STAGE, SV_LDG, I, (c + 1) * SV_R, I.m, gtid);
     cp_async_commit();
     const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE;
     const int rows = min(SV_R, I.m - c * SV_R);
@@ -126,20 +151,20 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
     }
   }
   cp_async_wait<0>();
-  __syncthreads();  // every warp is done with the stages: Hs (aliased onto stages 1..2) may be written
+  gsync(g);  // every warp is done with the stages: Hs (aliased onto the ring) may be written
 #pragma unroll
   for (int u = 0; u < 4; ++u)
 #pragma unroll
     for (int t = 0; t < 2; ++t)
       Hs[(8 * ti + lr) * SV_HLD + 8 * u + 2 * lk + t] = make_double2(cre[u][t], cim[u][t]);
-  __syncthreads();
+  gsync(g);
   // exact Hermitian symmetry from the upper triangle (the quick test and the rotations read p < q only)
-  for (int idx = threadIdx.x; idx < SV_W * SV_W; idx += U1_SVD_THREADS) {
+  for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
     const int p = idx >> 5, q = idx & 31;
     if (p > q) { const cplx v = Hs[q * SV_HLD + p]; Hs[p * SV_HLD + q] = make_double2(v.x, -v.y); }
     else if (p == q) Hs[p * SV_HLD + p].y = 0.0;
   }
-  __syncthreads();
+  gsync(g);
 }
 
 // pivot k of round t of the round-robin tournament over np2 players (not ordered: consecutive k give consecutive
@@ -165,10 +190,10 @@ __device__ __forceinline__ double rcp_approx(double x) { double y; asm("rcp.appr
 // to shrink the off-diagonal entry; the iteration is self-correcting), the normalisation is done in full precision so
 // that R is unitary to rounding whatever tau is.  The columns of R are swapped where needed so that the larger norm
 // ends up in the column with the lower index (de Rijk).
-__device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int* srot, int hp, double tol2, int* inner) {
-  const int tid = threadIdx.x;
+__device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int* srot, int hp, double tol2, int* inner, int inner_max, int g, int gtid) {
+  const int tid = gtid;
   const int np2 = 2 * hp;
-  for (int idx = tid; idx < SV_W * SV_QLD; idx += U1_SVD_THREADS) {
+  for (int idx = tid; idx < SV_W * SV_QLD; idx += SV_GROUP) {
     const int c = idx / SV_QLD, r = idx - c * SV_QLD;
     Qt[idx] = make_double2(r == c ? 1.0 : 0.0, 0.0);
   }
@@ -177,13 +202,13 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int*
   int uki[2], ukj[2];
 #pragma unroll
   for (int x = 0; x < 2; ++x) {
-    int u = tid + x * U1_SVD_THREADS, ki = 0;
+    int u = tid + x * SV_GROUP, ki = 0;
     if (u >= nunit) { uki[x] = -1; ukj[x] = 0; continue; }
     while (u >= hp - ki) { u -= hp - ki; ++ki; }
     uki[x] = ki; ukj[x] = ki + u;
   }
-  __syncthreads();
-  for (int sw = 0; sw < SV_INNER_MAX; ++sw) {
+  gsync(g);
+  for (int sw = 0; sw < inner_max; ++sw) {
     double mymax = 0.0;
     int sweep_any = 0;
     for (int t = 0; t < np2 - 1; ++t) {
@@ -229,7 +254,7 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int*
         pivot(t, max(uki[x], 0), np2, &pi[x], &qi[x]);
         pivot(t, ukj[x], np2, &pj[x], &qj[x]);
       }
-      const int any = __syncthreads_or(rot);
+      const int any = gsync_or(g, rot);
       if (!any) continue;  // nobody rotated in this round (uniform branch)
       sweep_any = 1;
 #pragma unroll
@@ -242,10 +267,10 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int*
         const cplx b10 = H[qi[x] * SV_HLD + pj[x]], b11 = H[qi[x] * SV_HLD + qj[x]];
         if (!(srot[ki] | srot[kj])) continue;  // both pivots idle
         // T = B Rj ; B' = Ri^H T
-        const cplx t00 = cadd(cmul(b00, j00), cmul(b01, j10)), t01 = cadd(cmul(b00, j01), cmul(b01, j11));
-        const cplx t10 = cadd(cmul(b10, j00), cmul(b11, j10)), t11 = cadd(cmul(b10, j01), cmul(b11, j11));
-        cplx n00 = cadd(cmulc(i00, t00), cmulc(i10, t10)), n01 = cadd(cmulc(i00, t01), cmulc(i10, t11));
-        cplx n10 = cadd(cmulc(i01, t00), cmulc(i11, t10)), n11 = cadd(cmulc(i01, t01), cmulc(i11, t11));
+        const cplx t00 = cdot2(b00, j00, b01, j10), t01 = cdot2(b00, j01, b01, j11);
+        const cplx t10 = cdot2(b10, j00, b11, j10), t11 = cdot2(b10, j01, b11, j11);
+        cplx n00 = cdot2c(i00, t00, i10, t10), n01 = cdot2c(i00, t01, i10, t11);
+        cplx n10 = cdot2c(i01, t00, i11, t10), n11 = cdot2c(i01, t01, i11, t11);
         if (ki == kj) {  // the pivot block itself: diagonal by construction
           n00.y = 0.0; n11.y = 0.0;
           n01 = make_double2(0.0, 0.0); n10 = n01;
@@ -257,7 +282,7 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int*
         }
       }
       // Q rows (rp, rp + hp), columns (pj, qj):  Q' = Q Rj ; Qt is column-major, consecutive threads take consecutive rows
-      for (int u = tid; u < hp * hp; u += U1_SVD_THREADS) {
+      for (int u = tid; u < hp * hp; u += SV_GROUP) {
         const int kj = u / hp, rp = u - kj * hp;
         int pc, qc;
         pivot(t, kj, np2, &pc, &qc);
@@ -266,23 +291,23 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int*
         cplx* cp = Qt + pc * SV_QLD + rp;
         cplx* cq = Qt + qc * SV_QLD + rp;
         const cplx q00 = cp[0], q01 = cq[0], q10 = cp[hp], q11 = cq[hp];
-        cp[0] = cadd(cmul(q00, j00), cmul(q01, j10));
-        cq[0] = cadd(cmul(q00, j01), cmul(q01, j11));
-        cp[hp] = cadd(cmul(q10, j00), cmul(q11, j10));
-        cq[hp] = cadd(cmul(q10, j01), cmul(q11, j11));
+        cp[0] = cdot2(q00, j00, q01, j10);
+        cq[0] = cdot2(q00, j01, q01, j11);
+        cp[hp] = cdot2(q10, j00, q11, j10);
+        cq[hp] = cdot2(q10, j01, q11, j11);
       }
-      __syncthreads();
+      gsync(g);
     }
     if (!sweep_any) break;
     ++*inner;
-    if (!__syncthreads_or(mymax > SV_QUAD)) break;
+    if (!gsync_or(g, mymax > SV_QUAD)) break;
   }
 }
 
 // ---- phase 3: [Pa Pb] <- [Pa Pb] Q over all mt rows.  Warp w owns tile column w (8 columns) and all row tiles
 // of each 32-row chunk; its 32 x 8 slice of Q lives in registers as 8 B fragments.
-__device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const Item& I) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+__device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const Item& I, int g, int gtid) {
+  const int lane = gtid & 31, warp = gtid >> 5;
   const int tj = warp;
   const int lr = lane >> 2, lk = lane & 3;
   double bre[8], bim[8];
@@ -291,7 +316,7 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
     const cplx v = Qt[(8 * tj + lr) * SV_QLD + 4 * ks + lk];   // Q[k][j], k = 4 ks + lk, j = 8 tj + lr
     bre[ks] = v.x; bim[ks] = v.y;
   }
-  __syncthreads();  // Q (aliased onto stages 1..2) is in registers everywhere: the ring may be refilled
+  gsync(g);  // Q (aliased onto the ring) is in registers everywhere: the ring may be refilled
   // the two output columns of this lane
   long long gcol[2]; bool cok[2];
 #pragma unroll
@@ -301,14 +326,12 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
     gcol[t] = (j < U1_PB ? I.ca + j : I.cb + j - U1_PB) * (long long)I.mt;
   }
   const int nch = (I.mt + SV_R - 1) / SV_R;
-  load_chunk(stages, SV_LDU, I, 0, I.mt);
-  cp_async_commit();
-  if (nch > 1) load_chunk(stages + SV_STAGE, SV_LDU, I, SV_R, I.mt);
+  load_chunk(stages, SV_LDU, I, 0, I.mt, gtid);
   cp_async_commit();
   for (int c = 0; c < nch; ++c) {
-    cp_async_wait<1>();
-    __syncthreads();
-    if (c + 2 < nch) load_chunk(stages + ((c + 2) % SV_NSTAGE) * SV_STAGE, SV_LDU, I, (c + 2) * SV_R, I.mt);
+    cp_async_wait<0>();
+    gsync(g);  // chunk c has landed for everybody, and everybody is done with chunk c - 1: its stage may be refilled
+    if (c + 1 < nch) load_chunk(stages + ((c + 1) % SV_NSTAGE) * SV_STAGE, SV_LDU, I, (c + 1) * SV_R, I.mt, gtid);
     cp_async_commit();
     const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE;
     const int row0 = c * SV_R;
@@ -334,21 +357,22 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
     }
   }
   cp_async_wait<0>();
-  __syncthreads();
+  gsync(g);
 }
 
-__global__ void __launch_bounds__(U1_SVD_THREADS, 4) svd_kernel(DevState S, Plan P) {
+__global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S, Plan P, int inner_max) {
   extern __shared__ __align__(16) unsigned char smraw[];
-  cplx* stages = reinterpret_cast<cplx*>(smraw);
-  cplx* Hs = stages + SV_STAGE;                    // [32*33], aliased onto stages 1..2 (idle during the EVD)
-  cplx* Qs = Hs + SV_W * SV_HLD;                   // [32*36], transposed
-  __shared__ cplx Rm[U1_PB][4];
-  __shared__ int srot[U1_PB];
   __shared__ unsigned s_ticket;
+  const int tid = threadIdx.x, g = tid / SV_GROUP, gtid = tid % SV_GROUP;
+  cplx* stages = reinterpret_cast<cplx*>(smraw + (size_t)g * SV_GROUP_BYTES);
+  cplx* Hs = stages;                               // [32*33], aliased onto the ring (idle during the EVD)
+  cplx* Qs = Hs + SV_W * SV_HLD;                   // [32*36], transposed
+  cplx (*Rm)[4] = reinterpret_cast<cplx (*)[4]>(Qs + SV_W * SV_QLD);   // [16][4] rotations of the current EVD round
+  int* srot = reinterpret_cast<int*>(Rm + U1_PB);  // [16]
+  static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD + U1_PB * 4) * 16 + U1_PB * 4, "EVD buffers must fit the idle stages");
   cg::grid_group grid = cg::this_grid();
   const int nblk = P.cnt[0], npair = P.cnt[1], maxP = P.cnt[3];
   const int rounds = max(maxP - 1, 1);
-  const int tid = threadIdx.x;
   unsigned base = 0;
   unsigned* ticket = reinterpret_cast<unsigned*>(P.cnt + 6);
   int sweep = 0;
@@ -357,65 +381,79 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, 4) svd_kernel(DevState S, Plan
     int n_rot = 0, n_inner = 0;
     for (int t = 0; t < rounds; ++t) {
       for (;;) {
+        // four consecutive items (same sector, as a rule) per CTA, one per group; the groups run the three phases in
+        // lock step so that the latency-bound EVDs never share the FP64 pipe with another group's DMMA stream
         __syncthreads();
-        if (tid == 0) s_ticket = atomicAdd(ticket, 1u) - base;
+        if (tid == 0) s_ticket = atomicAdd(ticket, (unsigned)SV_NGROUP) - base;
         __syncthreads();
-        const unsigned it = s_ticket;
-        if (it >= (unsigned)npair) break;
-        const int e = P.pitem_e[it], k = P.pitem_k[it];
-        if (sweep > 0 && __ldcg(&P.flags[e * U1_MAXSWEEP + sweep - 1]) == 0) continue;  // sector converged
-        const int r = P.rows[e], q = P.cols[e];
+        const unsigned it0 = s_ticket;
+        if (it0 >= (unsigned)npair) break;
+        const unsigned it = it0 + g;
+        bool have = it < (unsigned)npair;
         Item I;
-        I.m = max(r, q);
-        const int n = min(r, q);
-        I.mt = I.m + n;
-        const int np = u1_ceil_div(n, U1_PB);
-        const int np2 = np + (np & 1);
-        if (t >= max(np2 - 1, 1)) continue;
-        int pa, pb;
-        rr_pair(t, k, max(np2, 2), &pa, &pb);
-        if (pb >= np && np > 1) continue;  // bye (odd number of panels)
-        I.W = P.W + P.goff[e];
-        I.ca = pa * U1_PB; I.na = min(U1_PB, n - I.ca);
-        I.cb = pb * U1_PB; I.nb = pb < np ? min(U1_PB, n - I.cb) : 0;
-        const double tol = 8.0 * 1.1102230246251565e-16 * sqrt((double)I.m);
-        I.tol2 = tol * tol;
-        gram_phase(stages, Hs, I);
-        // quick test, same entries and arithmetic as the rotations: anything to do?
-        int todo = 0;
-        for (int idx = tid; idx < SV_W * SV_W; idx += U1_SVD_THREADS) {
-          const int p = idx >> 5, qq = idx & 31;
-          if (p < qq) {
-            const double a = Hs[p * SV_HLD + p].x, b = Hs[qq * SV_HLD + qq].x;
-            const cplx g = Hs[p * SV_HLD + qq];
-            const double ab = a * b;
-            todo |= (ab > 0.0 && g.x * g.x + g.y * g.y > I.tol2 * ab) ? 1 : 0;
-          }
+        int e = 0;
+        if (have) {
+          e = P.pitem_e[it];
+          const int k = P.pitem_k[it];
+          have = !(sweep > 0 && __ldcg(&P.flags[e * U1_MAXSWEEP + sweep - 1]) == 0);  // sector converged
+          const int r = P.rows[e], q = P.cols[e];
+          I.m = max(r, q);
+          const int n = min(r, q);
+          I.mt = I.m + n;
+          const int np = u1_ceil_div(n, U1_PB);
+          const int np2 = np + (np & 1);
+          if (t >= max(np2 - 1, 1)) have = false;
+          int pa, pb;
+          rr_pair(min(t, max(np2 - 2, 0)), k, max(np2, 2), &pa, &pb);
+          if (pb >= np && np > 1) have = false;  // bye (odd number of panels)
+          I.W = P.W + P.goff[e];
+          I.ca = pa * U1_PB; I.na = min(U1_PB, n - I.ca);
+          I.cb = pb * U1_PB; I.nb = pb < np ? min(U1_PB, n - I.cb) : 0;
+          const double tol = 8.0 * 1.1102230246251565e-16 * sqrt((double)I.m);
+          I.tol2 = tol * tol;
         }
-        if (!__syncthreads_or(todo)) continue;
-        if (tid == 0) P.flags[e * U1_MAXSWEEP + sweep] = 1;
+        int todo = 0;
+        if (have) {
+          gram_phase(stages, Hs, I, g, gtid);
+          // quick test, same entries and arithmetic as the rotations: anything to do?
+          for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
+            const int p = idx >> 5, qq = idx & 31;
+            if (p < qq) {
+              const double a = Hs[p * SV_HLD + p].x, b = Hs[qq * SV_HLD + qq].x;
+              const cplx gg = Hs[p * SV_HLD + qq];
+              const double ab = a * b, g2 = gg.x * gg.x + gg.y * gg.y;
+              todo |= (ab > 0.0 && g2 > I.tol2 * ab && g2 > 1e-290) ? 1 : 0;
+            }
+          }
+          todo = gsync_or(g, todo);
+          if (todo && gtid == 0) P.flags[e * U1_MAXSWEEP + sweep] = 1;
+        }
+        __syncthreads();
         int inner = 0;
-        evd_phase(Hs, Qs, Rm, srot, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner);
-        update_phase(stages, Qs, I);
-        n_rot += 1; n_inner += inner;
+        if (todo) evd_phase(Hs, Qs, Rm, srot, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
+        __syncthreads();
+        if (todo) {
+          update_phase(stages, Qs, I, g, gtid);
+          if (gtid == 0) { n_rot += 1; n_inner += inner; }
+        }
       }
-      base += (unsigned)npair + gridDim.x;
+      base += (unsigned)SV_NGROUP * ((unsigned)(npair + SV_NGROUP - 1) / SV_NGROUP + gridDim.x);
       grid.sync();
     }
     // ---- convergence: stop when no sector rotated in this sweep
     int any = 0;
     for (int bi = tid; bi < nblk; bi += U1_SVD_THREADS) any += __ldcg(&P.flags[P.blk[bi] * U1_MAXSWEEP + sweep]);
-    const int nact = __syncthreads_count(any);  // (threads that saw an active sector; exact count below)
-    if (tid == 0) {  // trace of this launch (u1mps_svd_trace)
-      if (n_rot) { atomicAdd((unsigned long long*)&P.trace[1 + U1_MAXSWEEP + sweep], (unsigned long long)n_rot);
-                   atomicAdd((unsigned long long*)&P.trace[1 + 2 * U1_MAXSWEEP + sweep], (unsigned long long)n_inner); }
-      if (blockIdx.x == 0) {
-        long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
-        P.trace[1 + sweep] = t1;
-        int act = 0;
-        for (int bi = 0; bi < nblk; ++bi) act += __ldcg(&P.flags[P.blk[bi] * U1_MAXSWEEP + sweep]);
-        P.trace[1 + 3 * U1_MAXSWEEP + sweep] = act;
-      }
+    const int nact = __syncthreads_count(any);
+    if (gtid == 0 && n_rot) {  // trace of this launch (u1mps_svd_trace)
+      atomicAdd((unsigned long long*)&P.trace[1 + U1_MAXSWEEP + sweep], (unsigned long long)n_rot);
+      atomicAdd((unsigned long long*)&P.trace[1 + 2 * U1_MAXSWEEP + sweep], (unsigned long long)n_inner);
+    }
+    if (tid == 0 && blockIdx.x == 0) {
+      long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+      P.trace[1 + sweep] = t1;
+      int act = 0;
+      for (int bi = 0; bi < nblk; ++bi) act += __ldcg(&P.flags[P.blk[bi] * U1_MAXSWEEP + sweep]);
+      P.trace[1 + 3 * U1_MAXSWEEP + sweep] = act;
     }
     if (nact == 0) { ++sweep; break; }
   }
@@ -490,7 +528,8 @@ cudaError_t u1_svd_configure(int* grid, int* smem_bytes, int sms) {
 cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
   (void)G;
   DevState s = S; Plan p = P;
-  void* args[] = {&s, &p};
+  static int inner_max = getenv("U1MPS_INNER_MAX") ? atoi(getenv("U1MPS_INNER_MAX")) : SV_INNER_MAX;
+  void* args[] = {&s, &p, &inner_max};
   L.prof->begin(U1_ST_SVD, L.stream);
   cudaError_t err = cudaLaunchCooperativeKernel((void*)svd_kernel, dim3(L.svd_grid), dim3(U1_SVD_THREADS), args,
                                                 (size_t)L.svd_smem, L.stream);
