@@ -5,6 +5,7 @@
 #include "common.cuh"
 
 #define PLAN_THREADS 1024
+#define U1_MAXPANELS (U1MPS_SORT_MAX / U1_PB)   // panels of the largest sector (n <= chi <= 4096)
 
 // Exclusive scan of f(0..L-1) into out[0..L] (out[L] = total) by one CTA.
 template <typename T, typename F>
@@ -32,6 +33,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
   __shared__ long long shl[PLAN_THREADS];
   __shared__ int shi[PLAN_THREADS];
   __shared__ int shmax;
+  __shared__ int cls_count[U1_MAXPANELS + 1], cls_fill[U1_MAXPANELS + 1], cls_base[U1_MAXPANELS + 1];
   const int NC = S.NC, d = S.d, E = G * NC, t = threadIdx.x;
   if (t == 0) shmax = 0;
   // (i)-(iii) rows(c), cols(c) of every candidate centre charge
@@ -88,24 +90,36 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
     if (min(P.rows[e], P.cols[e]) > 0) P.blk[P.tmpa[e]] = e;
   if (t == 0) P.cnt[0] = P.tmpa[E];
   __syncthreads();
-  // pair items: (p+1)/2 panel pairs per round of the round-robin tournament; a single panel is one item
-  block_excl_scan<int>([&](int e) { int p = panels(e); return (p + 1) / 2; }, P.tmpa, E, shi);
+  // pair items: (p+1)/2 panel pairs per round of the round-robin tournament; a single panel is one item.
+  // Items are listed by descending panel count (longest first): the a3 work queue hands them out in this order,
+  // so that the stragglers of a round are its cheapest items.
+  for (int i = t; i <= U1_MAXPANELS; i += PLAN_THREADS) { cls_count[i] = 0; cls_fill[i] = 0; }
+  __syncthreads();
+  for (int e = t; e < E; e += PLAN_THREADS) {
+    const int p = panels(e);
+    if (p > 0) atomicAdd(&cls_count[min(p, U1_MAXPANELS)], (p + 1) / 2);
+  }
+  __syncthreads();
   if (t == 0) {
-    P.cnt[1] = P.tmpa[E];
+    int run = 0;
+    for (int key = U1_MAXPANELS; key >= 1; --key) { cls_base[key] = run; run += cls_count[key]; }
+    cls_base[0] = run;  // total
+    P.cnt[1] = run;
     P.cnt[4] = P.t2pref[E * dd];
     P.cnt[5] = P.t5pref[E * 2];
     P.cnt[6] = 0;
-    if (P.tmpa[E] > P.itemcap) atomicExch(S.err, U1_ERR_WORKSPACE);
+    if (run > P.itemcap) atomicExch(S.err, U1_ERR_WORKSPACE);
   }
   __syncthreads();
-  const bool ok = P.tmpa[E] <= P.itemcap;
+  const bool ok = cls_base[0] <= P.itemcap;
   int mymax = 0;
   for (int e = t; e < E; e += PLAN_THREADS) {
     const int p = panels(e);
     if (p == 0 || !ok) continue;
     mymax = max(mymax, p + (p & 1));
-    const int np = (p + 1) / 2;
-    for (int k = 0; k < np; ++k) { P.pitem_e[P.tmpa[e] + k] = e; P.pitem_k[P.tmpa[e] + k] = k; }
+    const int np = (p + 1) / 2, key = min(p, U1_MAXPANELS);
+    const int off = cls_base[key] + atomicAdd(&cls_fill[key], np);
+    for (int k = 0; k < np; ++k) { P.pitem_e[off + k] = e; P.pitem_k[off + k] = k; }
   }
   atomicMax(&shmax, mymax);
   for (int i = t; i < E * U1_MAXSWEEP; i += PLAN_THREADS) P.flags[i] = 0;

@@ -30,7 +30,7 @@ namespace cg = cooperative_groups;
 #define SV_NSTAGE 2
 #define SV_HLD 33                    // leading dimension of the 32 x 32 Gram matrix (row-major)
 #define SV_QLD 36                    // leading dimension of the transposed eigenvector matrix Qt (4 mod 8: B fragments)
-#define SV_INNER_MAX 3               // inner EVD sweeps per item (the outer iteration finishes the job)
+#define SV_INNER_MAX 2               // inner EVD sweeps per item (the outer iteration finishes the job; measured best of 1..4)
 #define SV_QUAD 1e-14                // stop the inner EVD after a sweep whose largest relative off-diagonal^2 was below this
 #define SV_GROUP 128                 // threads per pair item; a CTA runs U1_SVD_THREADS / SV_GROUP = 4 items in lock-stepped phases
 #define SV_NGROUP (U1_SVD_THREADS / SV_GROUP)
@@ -117,13 +117,21 @@ __device__ __forceinline__ void load_chunk(cplx* st, int ld, const Item& I, int 
   }
 }
 
-// ---- phase 1: H = P^H P over rows [0, m).  Warp w owns tile row w of the 4 x 4 tiles (8 x 8 each).
+// ---- phase 1: H = P^H P over rows [0, m).  H is Hermitian: only the 10 tiles (8 x 8 each) of the upper triangle of
+// the 4 x 4 tile grid are computed, 3 + 3 + 2 + 2 per warp: warp 0 (0,0) (0,1) (0,2); warp 1 (3,0) (3,1) (3,2), stored
+// as the conjugate transposes (0,3) (1,3) (2,3); warp 2 (1,1) (1,2); warp 3 (2,2) (3,3).
 __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I, int g, int gtid) {
-  const int lane = gtid & 31, ti = gtid >> 5;
+  const int lane = gtid & 31, warp = gtid >> 5;
   const int lr = lane >> 2, lk = lane & 3;
-  double cre[4][2], cim[4][2];
+  // tile slots of this warp: (ta[u], tb[u]), u < nt
+  const int nt = warp < 2 ? 3 : 2;
+  int ta[3], tb[3];
+  ta[0] = warp == 0 ? 0 : warp == 1 ? 3 : warp == 2 ? 1 : 2;  tb[0] = warp == 0 ? 0 : warp == 1 ? 0 : warp == 2 ? 1 : 2;
+  ta[1] = warp == 0 ? 0 : warp == 1 ? 3 : warp == 2 ? 1 : 3;  tb[1] = warp == 0 ? 1 : warp == 1 ? 1 : warp == 2 ? 2 : 3;
+  ta[2] = warp == 0 ? 0 : 3;                                   tb[2] = 2;
+  double cre[3][2], cim[3][2];
 #pragma unroll
-  for (int u = 0; u < 4; ++u) { cre[u][0] = cre[u][1] = 0.0; cim[u][0] = cim[u][1] = 0.0; }
+  for (int u = 0; u < 3; ++u) { cre[u][0] = cre[u][1] = 0.0; cim[u][0] = cim[u][1] = 0.0; }
   const int nch = (I.m + SV_R - 1) / SV_R;
   load_chunk(stages, SV_LDG, I, 0, I.m, gtid);
   cp_async_commit();
@@ -132,31 +140,42 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
     gsync(g);  // chunk c has landed for everybody, and everybody is done with chunk c - 1: its stage may be refilled
     if (c + 1 < nch) load_chunk(stages + ((c + 1) % SV_NSTAGE) * SV_STAGE, SV_LDG, I, (c + 1) * SV_R, I.m, gtid);
     cp_async_commit();
-    const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE;
+    const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE + lr * SV_LDG + lk;
     const int rows = min(SV_R, I.m - c * SV_R);
     const int nk = (rows + 3) >> 2;
-    const cplx* pa = st + (8 * ti + lr) * SV_LDG + lk;
-    const cplx* pb = st + lr * SV_LDG + lk;
+    const cplx* pa0 = st + 8 * ta[0] * SV_LDG;   // slots 0 and 2 (if any) share the A tile of slot 0 or 1
+    const cplx* pa1 = st + 8 * ta[1] * SV_LDG;
+    const cplx* pb0 = st + 8 * tb[0] * SV_LDG;
+    const cplx* pb1 = st + 8 * tb[1] * SV_LDG;
+    const cplx* pb2 = st + 8 * tb[2] * SV_LDG;
 #pragma unroll 2
     for (int ks = 0; ks < nk; ++ks) {
-      const cplx a = pa[4 * ks];
-      const double nai = -a.y;
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const cplx b = pb[u * 8 * SV_LDG + 4 * ks];
-        // conj(a) * b : re = ar br + ai bi ; im = ar bi - ai br
-        dmma(cre[u][0], cre[u][1], a.x, b.x); dmma(cre[u][0], cre[u][1], a.y, b.y);
-        dmma(cim[u][0], cim[u][1], a.x, b.y); dmma(cim[u][0], cim[u][1], nai, b.x);
+      const cplx a0 = pa0[4 * ks], a1 = pa1[4 * ks], b0 = pb0[4 * ks], b1 = pb1[4 * ks];
+      // conj(a) * b : re = ar br + ai bi ; im = ar bi - ai br
+      dmma(cre[0][0], cre[0][1], a0.x, b0.x); dmma(cre[0][0], cre[0][1], a0.y, b0.y);
+      dmma(cim[0][0], cim[0][1], a0.x, b0.y); dmma(cim[0][0], cim[0][1], -a0.y, b0.x);
+      dmma(cre[1][0], cre[1][1], a1.x, b1.x); dmma(cre[1][0], cre[1][1], a1.y, b1.y);
+      dmma(cim[1][0], cim[1][1], a1.x, b1.y); dmma(cim[1][0], cim[1][1], -a1.y, b1.x);
+      if (nt == 3) {  // warp-uniform; the A tile of slot 2 is that of slot 0
+        const cplx b2 = pb2[4 * ks];
+        dmma(cre[2][0], cre[2][1], a0.x, b2.x); dmma(cre[2][0], cre[2][1], a0.y, b2.y);
+        dmma(cim[2][0], cim[2][1], a0.x, b2.y); dmma(cim[2][0], cim[2][1], -a0.y, b2.x);
       }
     }
   }
   cp_async_wait<0>();
   gsync(g);  // every warp is done with the stages: Hs (aliased onto the ring) may be written
 #pragma unroll
-  for (int u = 0; u < 4; ++u)
+  for (int u = 0; u < 3; ++u) {
+    if (u < nt) {
 #pragma unroll
-    for (int t = 0; t < 2; ++t)
-      Hs[(8 * ti + lr) * SV_HLD + 8 * u + 2 * lk + t] = make_double2(cre[u][t], cim[u][t]);
+      for (int t = 0; t < 2; ++t) {
+        const int r = 8 * ta[u] + lr, cidx = 8 * tb[u] + 2 * lk + t;
+        if (warp == 1) Hs[cidx * SV_HLD + r] = make_double2(cre[u][t], -cim[u][t]);   // tile (3, j) -> (j, 3)
+        else Hs[r * SV_HLD + cidx] = make_double2(cre[u][t], cim[u][t]);
+      }
+    }
+  }
   gsync(g);
   // exact Hermitian symmetry from the upper triangle (the quick test and the rotations read p < q only)
   for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
@@ -181,45 +200,76 @@ __device__ __forceinline__ double rsqrt_approx(double x) { double y; asm("rsqrt.
 __device__ __forceinline__ double rcp_approx(double x) { double y; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
 
 // ---- phase 2: two-sided Jacobi EVD of the Hermitian H (2*hp x 2*hp, hp = 16 or 8 pivots per round), Qt (stored
-// transposed) accumulates the rotations; both in place in shared memory: in a round the 2 x 2 unit (rows of pivot ki,
-// columns of pivot kj) is read and written by one thread only.  H stays exactly Hermitian: only units ki <= kj are
-// computed, each written together with its mirror image.
-// Rotation of the pivot (p, q) (a scalar one-sided rotation of columns p, q, whose Gram entries are a = h_pp, b = h_qq,
-// g = h_pq):  zeta = (b - a) / (2|g|), t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)), tau = t g/|g|,
-// R = [[1, tau], [-conj(tau), 1]] / sqrt(1 + |tau|^2).  tau comes from the ~20-bit MUFU reciprocal / rsqrt (it only has
-// to shrink the off-diagonal entry; the iteration is self-correcting), the normalisation is done in full precision so
-// that R is unitary to rounding whatever tau is.  The columns of R are swapped where needed so that the larger norm
-// ends up in the column with the lower index (de Rijk).
-__device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int* srot, int hp, double tol2, int* inner, int inner_max, int g, int gtid) {
+// transposed) accumulates the rotations; both in place in shared memory.
+// Round t of a sweep rotates the hp disjoint pivots (p_k, q_k) of the round-robin tournament.  Rotation of a pivot
+// (p, q) (= a scalar one-sided rotation of columns p, q, whose Gram entries are a = h_pp, b = h_qq, g = h_pq):
+//   zeta = (b - a) / (2|g|), t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)), tau = t g/|g|, cs = 1/sqrt(1 + |tau|^2),
+//   s = cs tau,  R = [[cs, s], [-conj(s), cs]].
+// tau comes from the ~20-bit MUFU reciprocal / rsqrt (it only has to shrink the off-diagonal entry; the iteration is
+// self-correcting), cs is computed in full precision so that R is unitary to rounding whatever tau is.  Where the
+// new norms would be out of order the two result columns are exchanged (de Rijk: the larger norm goes to the lower index).
+// Work split of a round: thread k < hp computes rotation k and rewrites its own 2 x 2 pivot block (closed form);
+// after the barrier every 2 x 2 unit (rows of pivot ki, columns of pivot kj, ki < kj) is read, rotated from both
+// sides and written, together with its mirror image, by one thread (H stays exactly Hermitian); the Q units
+// (two rows x the two columns of a pivot) likewise.  Pivot indices advance by one (mod 2hp - 1) per round.
+struct Rot { double cs, sr, si; int flag; };   // flag: 0 idle, 1 rotate, 3 rotate and exchange
+__device__ __forceinline__ Rot load_rot(const double4* Rm, int k) {
+  const double4 v = Rm[k];
+  Rot r; r.cs = v.x; r.sr = v.y; r.si = v.z; r.flag = (int)v.w;
+  return r;
+}
+// [x y] <- [x y] R :  x' = cs x - conj(s) y,  y' = s x + cs y
+__device__ __forceinline__ void rot_cols(cplx& x, cplx& y, const Rot& r) {
+  const cplx xn = make_double2(fma(-r.sr, y.x, fma(-r.si, y.y, r.cs * x.x)), fma(-r.sr, y.y, fma(r.si, y.x, r.cs * x.y)));
+  const cplx yn = make_double2(fma(r.sr, x.x, fma(-r.si, x.y, r.cs * y.x)), fma(r.sr, x.y, fma(r.si, x.x, r.cs * y.y)));
+  x = xn; y = yn;
+}
+// [x; y] <- R^H [x; y] :  x' = cs x - s y,  y' = conj(s) x + cs y
+__device__ __forceinline__ void rot_rows(cplx& x, cplx& y, const Rot& r) {
+  const cplx xn = make_double2(fma(-r.sr, y.x, fma(r.si, y.y, r.cs * x.x)), fma(-r.sr, y.y, fma(-r.si, y.x, r.cs * x.y)));
+  const cplx yn = make_double2(fma(r.sr, x.x, fma(r.si, x.y, r.cs * y.x)), fma(r.sr, x.y, fma(-r.si, x.x, r.cs * y.y)));
+  x = xn; y = yn;
+}
+__device__ __forceinline__ void advance(int& p, int& q, int k, int m) {  // pivot k of the next round
+  if (++p == m) p = 0;
+  if (k != 0 && ++q == m) q = 0;
+}
+
+__device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, int hp, double tol2, int* inner, int inner_max, int g, int gtid) {
   const int tid = gtid;
-  const int np2 = 2 * hp;
+  const int np2 = 2 * hp, m = np2 - 1;
   for (int idx = tid; idx < SV_W * SV_QLD; idx += SV_GROUP) {
     const int c = idx / SV_QLD, r = idx - c * SV_QLD;
     Qt[idx] = make_double2(r == c ? 1.0 : 0.0, 0.0);
   }
-  // H units of this thread: entries tid and tid + 128 of the row-major list of the upper triangle ki <= kj
-  const int nunit = hp * (hp + 1) / 2;
-  int uki[2], ukj[2];
-#pragma unroll
-  for (int x = 0; x < 2; ++x) {
-    int u = tid + x * SV_GROUP, ki = 0;
-    if (u >= nunit) { uki[x] = -1; ukj[x] = 0; continue; }
-    while (u >= hp - ki) { u -= hp - ki; ++ki; }
-    uki[x] = ki; ukj[x] = ki + u;
+  // this thread's H unit: entry tid of the row-major list of the strict upper triangle ki < kj
+  int uki = -1, ukj = 0;
+  {
+    int u = tid, ki = 0;
+    if (u < hp * (hp - 1) / 2) {
+      while (u >= hp - 1 - ki) { u -= hp - 1 - ki; ++ki; }
+      uki = ki; ukj = ki + 1 + u;
+    }
   }
+  // this thread's Q units: rows (rp, rp + hp) x pivots kq0 and kq0 + 8 (hp = 16), or pivot kq0 only (hp = 8, tid < 64)
+  const int rp = tid % hp, kq0 = tid / hp;
+  const int nq = (hp == U1_PB) ? 2 : (tid < hp * hp ? 1 : 0);
   gsync(g);
   for (int sw = 0; sw < inner_max; ++sw) {
     double mymax = 0.0;
     int sweep_any = 0;
-    for (int t = 0; t < np2 - 1; ++t) {
+    // pivots at round 0: (k, m - k) for k >= 1, (0, m) for k = 0
+    int pp = tid < hp ? tid : 0, pq = tid < hp ? m - tid : 0;                 // rotation owned by this thread (tid < hp)
+    int pi = max(uki, 0), qi = m - max(uki, 0), pj = ukj, qj = m - ukj;         // H unit
+    int pc0 = kq0, qc0 = m - kq0, pc1 = kq0 + 8, qc1 = m - kq0 - 8;            // Q units
+    for (int t = 0; t < m; ++t) {
       int rot = 0;
       if (tid < hp) {
-        int p, q;
-        pivot(t, tid, np2, &p, &q);
+        const int p = pp, q = pq;
         const double a = H[p * SV_HLD + p].x, b = H[q * SV_HLD + q].x;
-        const cplx g = H[p * SV_HLD + q];
-        const double g2 = g.x * g.x + g.y * g.y, ab = a * b;
-        cplx r00 = make_double2(1.0, 0.0), r01 = make_double2(0.0, 0.0), r10 = r01, r11 = r00;
+        const cplx gg = H[p * SV_HLD + q];
+        const double g2 = gg.x * gg.x + gg.y * gg.y, ab = a * b;
+        double4 out = make_double4(1.0, 0.0, 0.0, 0.0);
         if (ab > 0.0 && g2 > tol2 * ab && g2 > 1e-290) {
           rot = 1;
           mymax = fmax(mymax, g2 * rcp_approx(ab));
@@ -228,75 +278,71 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, cplx (*Rm)[4], int*
           const double z1 = fma(zeta, zeta, 1.0);
           const double tt = copysign(rcp_approx(fabs(zeta) + z1 * rsqrt_approx(z1)), zeta);
           const double ti = tt * iag;
-          const double tx = ti * g.x, ty = ti * g.y;           // tau
+          const double tx = ti * gg.x, ty = ti * gg.y;         // tau
           const double n2 = fma(tx, tx, fma(ty, ty, 1.0));
           double cs = rsqrt_approx(n2);                        // two Newton steps: full precision
           cs = fma(0.5 * cs, fma(-n2 * cs, cs, 1.0), cs);
           cs = fma(0.5 * cs, fma(-n2 * cs, cs, 1.0), cs);
           const double sr = cs * tx, si = cs * ty;
-          const double dn = tt * g2 * iag;                     // norms after the rotation: a - dn (column p), b + dn (column q)
-          const bool swp = (p < q) ? (a - dn < b + dn) : (b + dn < a - dn);
+          // the pivot block after the rotation, in closed form (x' = cs x - conj(s) y, y' = s x + cs y):
+          //   a' = cs^2 a + |s|^2 b - 2 cs Re(conj(s) g),  b' = |s|^2 a + cs^2 b + 2 cs Re(conj(s) g),
+          //   g' = x'^H y' = cs s (a - b) + cs^2 g - s^2 conj(g)
+          const double s2 = sr * sr + si * si, c2 = cs * cs;
+          const double cr = 2.0 * cs * (sr * gg.x + si * gg.y);
+          const double an = fma(c2, a, fma(s2, b, -cr)), bn = fma(s2, a, fma(c2, b, cr));
+          const double s2r = sr * sr - si * si, s2i = 2.0 * sr * si;   // s^2
+          const double gnx = fma(cs * sr, a - b, fma(c2, gg.x, -(s2r * gg.x + s2i * gg.y)));
+          const double gny = fma(cs * si, a - b, fma(c2, gg.y, -(s2i * gg.x - s2r * gg.y)));
+          const bool swp = (p < q) ? (an < bn) : (bn < an);
+          out = make_double4(cs, sr, si, swp ? 3.0 : 1.0);
           if (swp) {
-            r00 = make_double2(sr, si); r01 = make_double2(cs, 0.0);
-            r10 = make_double2(cs, 0.0); r11 = make_double2(-sr, si);
+            H[p * SV_HLD + p] = make_double2(bn, 0.0); H[q * SV_HLD + q] = make_double2(an, 0.0);
+            H[p * SV_HLD + q] = make_double2(gnx, -gny); H[q * SV_HLD + p] = make_double2(gnx, gny);
           } else {
-            r00 = make_double2(cs, 0.0); r01 = make_double2(sr, si);
-            r10 = make_double2(-sr, si); r11 = make_double2(cs, 0.0);
+            H[p * SV_HLD + p] = make_double2(an, 0.0); H[q * SV_HLD + q] = make_double2(bn, 0.0);
+            H[p * SV_HLD + q] = make_double2(gnx, gny); H[q * SV_HLD + p] = make_double2(gnx, -gny);
           }
         }
-        Rm[tid][0] = r00; Rm[tid][1] = r01; Rm[tid][2] = r10; Rm[tid][3] = r11;
-        srot[tid] = rot;
-      }
-      // pivots of this thread's units (integer work, overlaps the rotation parameters of warp 0)
-      int pi[2], qi[2], pj[2], qj[2];
-#pragma unroll
-      for (int x = 0; x < 2; ++x) {
-        pivot(t, max(uki[x], 0), np2, &pi[x], &qi[x]);
-        pivot(t, ukj[x], np2, &pj[x], &qj[x]);
+        Rm[tid] = out;
       }
       const int any = gsync_or(g, rot);
-      if (!any) continue;  // nobody rotated in this round (uniform branch)
-      sweep_any = 1;
-#pragma unroll
-      for (int x = 0; x < 2; ++x) {
-        const int ki = uki[x], kj = ukj[x];
-        if (ki < 0) continue;
-        const cplx j00 = Rm[kj][0], j01 = Rm[kj][1], j10 = Rm[kj][2], j11 = Rm[kj][3];
-        const cplx i00 = Rm[ki][0], i01 = Rm[ki][1], i10 = Rm[ki][2], i11 = Rm[ki][3];
-        const cplx b00 = H[pi[x] * SV_HLD + pj[x]], b01 = H[pi[x] * SV_HLD + qj[x]];
-        const cplx b10 = H[qi[x] * SV_HLD + pj[x]], b11 = H[qi[x] * SV_HLD + qj[x]];
-        if (!(srot[ki] | srot[kj])) continue;  // both pivots idle
-        // T = B Rj ; B' = Ri^H T
-        const cplx t00 = cdot2(b00, j00, b01, j10), t01 = cdot2(b00, j01, b01, j11);
-        const cplx t10 = cdot2(b10, j00, b11, j10), t11 = cdot2(b10, j01, b11, j11);
-        cplx n00 = cdot2c(i00, t00, i10, t10), n01 = cdot2c(i00, t01, i10, t11);
-        cplx n10 = cdot2c(i01, t00, i11, t10), n11 = cdot2c(i01, t01, i11, t11);
-        if (ki == kj) {  // the pivot block itself: diagonal by construction
-          n00.y = 0.0; n11.y = 0.0;
-          n01 = make_double2(0.0, 0.0); n10 = n01;
-          H[pi[x] * SV_HLD + pi[x]] = n00; H[pi[x] * SV_HLD + qi[x]] = n01; H[qi[x] * SV_HLD + pi[x]] = n10; H[qi[x] * SV_HLD + qi[x]] = n11;
-        } else {
-          H[pi[x] * SV_HLD + pj[x]] = n00; H[pi[x] * SV_HLD + qj[x]] = n01; H[qi[x] * SV_HLD + pj[x]] = n10; H[qi[x] * SV_HLD + qj[x]] = n11;
-          H[pj[x] * SV_HLD + pi[x]] = make_double2(n00.x, -n00.y); H[qj[x] * SV_HLD + pi[x]] = make_double2(n01.x, -n01.y);
-          H[pj[x] * SV_HLD + qi[x]] = make_double2(n10.x, -n10.y); H[qj[x] * SV_HLD + qi[x]] = make_double2(n11.x, -n11.y);
+      if (any) {  // uniform
+        sweep_any = 1;
+        if (uki >= 0) {
+          const Rot ri = load_rot(Rm, uki), rj = load_rot(Rm, ukj);
+          if (ri.flag | rj.flag) {
+            cplx b00 = H[pi * SV_HLD + pj], b01 = H[pi * SV_HLD + qj], b10 = H[qi * SV_HLD + pj], b11 = H[qi * SV_HLD + qj];
+            if (rj.flag) { rot_cols(b00, b01, rj); rot_cols(b10, b11, rj); }
+            if (ri.flag) { rot_rows(b00, b10, ri); rot_rows(b01, b11, ri); }
+            // exchanges are applied to the destinations
+            const int dpi = (ri.flag & 2) ? qi : pi, dqi = (ri.flag & 2) ? pi : qi;
+            const int dpj = (rj.flag & 2) ? qj : pj, dqj = (rj.flag & 2) ? pj : qj;
+            H[dpi * SV_HLD + dpj] = b00; H[dpi * SV_HLD + dqj] = b01; H[dqi * SV_HLD + dpj] = b10; H[dqi * SV_HLD + dqj] = b11;
+            H[dpj * SV_HLD + dpi] = make_double2(b00.x, -b00.y); H[dqj * SV_HLD + dpi] = make_double2(b01.x, -b01.y);
+            H[dpj * SV_HLD + dqi] = make_double2(b10.x, -b10.y); H[dqj * SV_HLD + dqi] = make_double2(b11.x, -b11.y);
+          }
         }
+#pragma unroll
+        for (int x = 0; x < 2; ++x) {
+          if (x < nq) {
+            const Rot rj = load_rot(Rm, kq0 + 8 * x);
+            if (rj.flag) {
+              const int pc = x ? pc1 : pc0, qc = x ? qc1 : qc0;
+              cplx* cp = Qt + pc * SV_QLD + rp;
+              cplx* cq = Qt + qc * SV_QLD + rp;
+              cplx q00 = cp[0], q01 = cq[0], q10 = cp[hp], q11 = cq[hp];
+              rot_cols(q00, q01, rj); rot_cols(q10, q11, rj);
+              cplx* dp = (rj.flag & 2) ? cq : cp;
+              cplx* dq = (rj.flag & 2) ? cp : cq;
+              dp[0] = q00; dq[0] = q01; dp[hp] = q10; dq[hp] = q11;
+            }
+          }
+        }
+        gsync(g);
       }
-      // Q rows (rp, rp + hp), columns (pj, qj):  Q' = Q Rj ; Qt is column-major, consecutive threads take consecutive rows
-      for (int u = tid; u < hp * hp; u += SV_GROUP) {
-        const int kj = u / hp, rp = u - kj * hp;
-        int pc, qc;
-        pivot(t, kj, np2, &pc, &qc);
-        const cplx j00 = Rm[kj][0], j01 = Rm[kj][1], j10 = Rm[kj][2], j11 = Rm[kj][3];
-        if (!srot[kj]) continue;
-        cplx* cp = Qt + pc * SV_QLD + rp;
-        cplx* cq = Qt + qc * SV_QLD + rp;
-        const cplx q00 = cp[0], q01 = cq[0], q10 = cp[hp], q11 = cq[hp];
-        cp[0] = cdot2(q00, j00, q01, j10);
-        cq[0] = cdot2(q00, j01, q01, j11);
-        cp[hp] = cdot2(q10, j00, q11, j10);
-        cq[hp] = cdot2(q10, j01, q11, j11);
-      }
-      gsync(g);
+      advance(pp, pq, tid, m);
+      advance(pi, qi, uki, m); advance(pj, qj, ukj, m);
+      advance(pc0, qc0, kq0, m); advance(pc1, qc1, kq0 + 8, m);
     }
     if (!sweep_any) break;
     ++*inner;
@@ -367,9 +413,8 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
   cplx* stages = reinterpret_cast<cplx*>(smraw + (size_t)g * SV_GROUP_BYTES);
   cplx* Hs = stages;                               // [32*33], aliased onto the ring (idle during the EVD)
   cplx* Qs = Hs + SV_W * SV_HLD;                   // [32*36], transposed
-  cplx (*Rm)[4] = reinterpret_cast<cplx (*)[4]>(Qs + SV_W * SV_QLD);   // [16][4] rotations of the current EVD round
-  int* srot = reinterpret_cast<int*>(Rm + U1_PB);  // [16]
-  static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD + U1_PB * 4) * 16 + U1_PB * 4, "EVD buffers must fit the idle stages");
+  double4* Rm = reinterpret_cast<double4*>(Qs + SV_W * SV_QLD);   // [16] rotations of the current EVD round
+  static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD) * 16 + U1_PB * 32, "EVD buffers must fit the idle stages");
   cg::grid_group grid = cg::this_grid();
   const int nblk = P.cnt[0], npair = P.cnt[1], maxP = P.cnt[3];
   const int rounds = max(maxP - 1, 1);
@@ -430,7 +475,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
         }
         __syncthreads();
         int inner = 0;
-        if (todo) evd_phase(Hs, Qs, Rm, srot, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
+        if (todo) evd_phase(Hs, Qs, Rm, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
         __syncthreads();
         if (todo) {
           update_phase(stages, Qs, I, g, gtid);
