@@ -158,7 +158,8 @@ def oracle_sample(w, n_gates, seed0=4242):
     cols = list(inputs.gate_columns(w, 1))
     total = 0.0
     for g in range(n_gates):
-        M, N, s, lam, gam = inputs.synthetic_gate_state(w.d, w.chi, SYNTH_R[w.index], seed=seed0 + g)
+        M, N, s, lam, gam = inputs.synthetic_gate_state(w.d, w.chi, SYNTH_R[w.index], seed=seed0 + g,
+                                                        profile=inputs.SATURATED_PROFILE.get(w.index))
         occ, left = [0] * M, N
         for i in range(M):
             occ[i] = min(w.d - 1, left)
@@ -181,6 +182,33 @@ def oracle_sample(w, n_gates, seed0=4242):
     return n_gates / total, total, cores
 
 
+def sample_profile(w):
+    prof = inputs.SATURATED_PROFILE.get(w.index)
+    if prof is not None:
+        return f"sector sizes {list(prof)} as measured on this workload's trajectory after {w.columns} columns"
+    return f"{SYNTH_R[w.index]} sectors, parabolic profile"
+
+
+def dist_max(values, world, device):
+    """Max over ranks of a list of floats (the timed regions); a plain identity for world == 1.
+    Used with NCCL tensors by the GPU arm and with gloo/CPU tensors by tests/test_bench_contract.py."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def svd_traffic_bytes():
+    """DRAM bytes (read + write) of ONE a3 launch from the committed ncu --set full capture, or None."""
+    try:
+        d = json.load(open(os.path.join(ROOT, "profiles", "svd_traffic.json")))
+        return float(d["dram_bytes_read"]) + float(d["dram_bytes_write"])
+    except Exception:
+        return None
+
+
 def run_reference(args, w):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -195,7 +223,7 @@ def run_reference(args, w):
         n_tot += sample_gates
     val = n_tot / t_tot
     sample = (f"{sample_gates} gates/step on seeded synthetic saturated-bond states (d={w.d}, chi={w.chi}, "
-              f"{SYNTH_R[w.index]} sectors, parabolic profile), numpy oracle")
+              f"{sample_profile(w)}), numpy oracle")
     print(json.dumps({
         "impl": "reference", "metric": "two-site U(1) gate updates/sec", "value": val, "unit": "gates/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
@@ -307,10 +335,7 @@ def run_ours(args, w):
     stats = gpu.last_stats()
     total_n = float(np.sum(n_k))
 
-    t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e = float(t[0]), float(t[1])
+    ms, ms_e2e = dist_max([ms, ms_e2e], world, "cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -332,7 +357,7 @@ def run_ours(args, w):
         rate, secs, cores = oracle_sample(w, args.cpu_gates)
         cpu = {"value": rate, "unit": "gates/s", "cores": cores, "kind": "oracle",
                "sample": f"{args.cpu_gates} gates on seeded synthetic saturated-bond states (d={w.d}, chi={w.chi}, "
-                         f"{SYNTH_R[w.index]} sectors, parabolic profile), {secs:.1f} s of numpy/LAPACK work"}
+                         f"{sample_profile(w)}), {secs:.1f} s of numpy/LAPACK work"}
 
     out = {
         "metric": "two-site U(1) gate updates/sec", "value": value, "unit": "gates/s", "n_gpus": world,
@@ -351,8 +376,10 @@ def run_ours(args, w):
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"kernel": "svd_kernel (a3)", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak, "traffic": None,
-                     "peak_source": "derived: 148 SMs x 64 FP64 FMA/clk x 2 x sm_max_mhz (no FP64 entry in MEASURED_PEAKS.json)",
+                     "frac": achieved / peak, "traffic": svd_traffic_bytes(),
+                     "peak_source": "derived: 148 SMs x 64 FP64 FMA/clk x 2 x sm_max_mhz (no FP64 entry in MEASURED_PEAKS.json; "
+                                    "the round-1 probe measured 36.8 DFMA / 37.06 DMMA TFLOP/s, DESIGN.md section 6)",
+                     "traffic_source": "profiles/svd_traffic.json (ncu --set full, one launch of the same workload)",
                      "flops": "useful SVD flops 4*min(14mn^2+8n^3, 6mn^2+20n^3) per block (SURVEY §8(d))",
                      "ms_per_launch": svd_ms / max(svd_n, 1), "launches": svd_n,
                      "share_of_step": svd_ms / ms if ms > 0 else None},

@@ -218,7 +218,12 @@ def parabolic_profile(chi: int, R: int) -> List[int]:
     return [int(v) for v in n]
 
 
-def synthetic_gate_state(d: int, chi: int, R: int, seed: int, decay: float = 0.97):
+# sector sizes of a saturated bond of config 3 (XXZ, chi = 1024) as measured on the trajectory after 50 layers
+# (DESIGN.md section 4); used so that the CPU-baseline sample has the block sizes of the real workload
+SATURATED_PROFILE = {3: (5, 32, 100, 195, 256, 229, 139, 54, 13, 1)}
+
+
+def synthetic_gate_state(d: int, chi: int, R: int, seed: int, decay: float = 0.97, profile=None):
     """Random three-bond neighbourhood for one gate on sites (2, 3) of a short chain (M >= 6).
 
     Returns (M, N, site, lam, gam): lam[k] = {c: descending positive vector} for bonds 2, 3, 4;
@@ -230,13 +235,16 @@ def synthetic_gate_state(d: int, chi: int, R: int, seed: int, decay: float = 0.9
     rng = np.random.default_rng(seed)
     site = 2
     step = max(1, d // 2)
-    N = R + 4 * step + 2
+    if profile is not None:
+        R = len(profile)
+    N0 = R + 4 * step + 2
+    first = {k: max(0, N0 - 2 - (k - 1) * step - R // 2 + 1) for k in (2, 3, 4)}
+    N = max(N0, first[2] + R - 1)          # every sector charge must lie in [0, N]
     M = max(6, -(-N // (d - 1)) + 1)
-    prof = parabolic_profile(chi, R)
+    prof = list(profile) if profile is not None else parabolic_profile(chi, R)
     lam, gam = {}, {}
     for k in (2, 3, 4):
-        c0 = N - 2 - (k - 1) * step - R // 2 + 1
-        c0 = max(0, c0)
+        c0 = first[k]
         lk = {}
         for x, n in enumerate(prof):
             v = np.sort(rng.uniform(0.5, 1.0, n) * decay ** np.arange(n))[::-1]
