@@ -2,20 +2,24 @@
 //   Theta(c)[rows of c_l, cols of c_r] = lamL[c_l] * ( sum_{c'} U[(c_l-c, c-c_r),(c_l-c', c'-c_r)]
 //                                         * Gamma^[s][c_l,c'] * lamC[c'] * Gamma^[s+1][c',c_r] ) * lamR[c_r]
 // One persistent grid walks the tile list built by the planner (variable-size sectors of all
-// gates of the chunk).  The U entry is a scalar per K-chunk (the delta functions of Eq.16 "tell us
+// gates of the chunk), 32 x 32 output tiles on FP64 tensor tiles (DMMA.8x8x4, 4 real MMAs per complex product).
+// The U entry is a scalar per K-chunk (the delta functions of Eq.16 "tell us
 // which entry of the unitary matrix to look up", L121), folded into the A operand together with
 // lambda^[k]; lambda^[k-1], lambda^[k+1] are applied in the epilogue.  The result is written straight
 // into the stacked column-major Jacobi matrix of the sector: Theta(c) if rows >= cols, else its
 // conjugate transpose, with the identity (accumulator of the right singular vectors) below it.
 #include "common.cuh"
 
-#define KC 16
-#define CT_THREADS 256
+#define KC 16          // K-chunk (columns of A / rows of B) per stage
+#define CT_THREADS 128 // 4 warps: warp w owns rows 8w..8w+7 of the 32 x 32 output tile (4 DMMA tiles of 8 x 8)
+#define CT_LD 34       // shared-memory leading dimension (complex elements), 2 mod 8: conflict-free LDS.128 fragments
 
 __device__ __forceinline__ cplx cmul(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-__device__ __forceinline__ void cfma(cplx& acc, cplx a, cplx b) {
-  acc.x = fma(a.x, b.x, acc.x); acc.x = fma(-a.y, b.y, acc.x);
-  acc.y = fma(a.x, b.y, acc.y); acc.y = fma(a.y, b.x, acc.y);
+
+// D(8x8) += A(8x4, row) * B(4x8, col), FP64 tensor tile (SASS: DMMA.8x8x4).
+// Fragments: a = A[lane>>2][lane&3], b = B[lane&3][lane>>2], c0/c1 = C[lane>>2][2*(lane&3) + 0/1].
+__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
 // largest idx in [0, n) with pref[idx] <= v  (pref non-decreasing, pref[0] = 0 <= v < pref[n])
@@ -29,12 +33,12 @@ __device__ __forceinline__ int upper_entry(const int* __restrict__ pref, int n, 
 }
 
 __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P, int G) {
-  __shared__ cplx As[KC][U1_TILE + 1];
-  __shared__ cplx Bs[KC][U1_TILE];
+  __shared__ __align__(16) cplx As[KC * CT_LD];   // As[k][a]: (u lamC[k]) A[a0 + a][k0 + k]
+  __shared__ __align__(16) cplx Bs[KC * CT_LD];   // Bs[k][b]: B[k0 + k][b0 + b]
   const int NC = S.NC, d = S.d, dd = d * d, N = S.N;
   const int nf = G * NC * dd;
   const int total = P.cnt[4];
-  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, lr = lane >> 2, lk = lane & 3;
   for (int tile = blockIdx.x; tile < total; tile += gridDim.x) {
     const int f = upper_entry(P.t2pref, nf, tile);
     const int e = f / dd, i = (f / d) % d, j = f % d;
@@ -50,8 +54,9 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P
     const cplx* Ug = P.U + (long long)g * dd * dd + (long long)(i * d + j) * dd;  // row (out_s = i, out_{s+1} = j)
     const cplx* gA = S.gam + (long long)s * S.gcap;
     const cplx* gB = S.gam + (long long)(s + 1) * S.gcap;
-    cplx acc[2][2];
-    acc[0][0] = acc[0][1] = acc[1][0] = acc[1][1] = make_double2(0.0, 0.0);
+    double cre[4][2], cim[4][2];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { cre[u][0] = cre[u][1] = 0.0; cim[u][0] = cim[u][1] = 0.0; }
     const int cplo = max(max(cr, cl - d + 1), 0), cphi = min(min(cl, cr + d - 1), N);
     for (int cp = cplo; cp <= cphi; ++cp) {  // old centre sectors c' (the alpha_k sum of Eq.16, sector by sector)
       const int nC = nbC[cp];
@@ -61,35 +66,54 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P
       const cplx* B = gB + S.gamoff[((long long)(s + 1) * NC + cp) * d + (cp - cr)];  // nC x nR
       const double* lamC = S.lam + (long long)(s + 1) * S.chi + S.ob[(long long)(s + 1) * NC + cp];
       for (int k0 = 0; k0 < nC; k0 += KC) {
-        __syncthreads();
-        {  // A tile: k fastest
+        // global -> registers (A: k fastest, B: b fastest: both coalesced), scale A by u lamC[k]
+        cplx ra[4], rb[4];
+        {
           const int k = tid & (KC - 1);
-          for (int a = tid / KC; a < U1_TILE; a += CT_THREADS / KC) {
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const int a = (tid >> 4) + 8 * x;
             cplx v = make_double2(0.0, 0.0);
             if (a0 + a < nL && k0 + k < nC) {
-              v = A[(long long)(a0 + a) * nC + k0 + k];
               const double l = lamC[k0 + k];
-              v = cmul(v, make_double2(u.x * l, u.y * l));
+              v = cmul(A[(long long)(a0 + a) * nC + k0 + k], make_double2(u.x * l, u.y * l));
             }
-            As[k][a] = v;
+            ra[x] = v;
           }
           const int b = tid & (U1_TILE - 1);
-          for (int kk = tid / U1_TILE; kk < KC; kk += CT_THREADS / U1_TILE) {
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const int kk = (tid >> 5) + 4 * x;
             cplx v = make_double2(0.0, 0.0);
             if (b0 + b < nR && k0 + kk < nC) v = B[(long long)(k0 + kk) * nR + b0 + b];
-            Bs[kk][b] = v;
+            rb[x] = v;
+          }
+        }
+        __syncthreads();  // the previous chunk has been consumed
+        {
+          const int k = tid & (KC - 1), b = tid & (U1_TILE - 1);
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            As[k * CT_LD + (tid >> 4) + 8 * x] = ra[x];
+            Bs[((tid >> 5) + 4 * x) * CT_LD + b] = rb[x];
           }
         }
         __syncthreads();
+        const int nk = (min(KC, nC - k0) + 3) >> 2;
+        for (int ks = 0; ks < nk; ++ks) {
+          const cplx av = As[(4 * ks + lk) * CT_LD + 8 * warp + lr];
+          const double nai = -av.y;
 #pragma unroll
-        for (int k = 0; k < KC; ++k) {
-          const cplx x0 = As[k][ty * 2], x1 = As[k][ty * 2 + 1];
-          const cplx y0 = Bs[k][tx * 2], y1 = Bs[k][tx * 2 + 1];
-          cfma(acc[0][0], x0, y0); cfma(acc[0][1], x0, y1);
-          cfma(acc[1][0], x1, y0); cfma(acc[1][1], x1, y1);
+          for (int t = 0; t < 4; ++t) {
+            const cplx bv = Bs[(4 * ks + lk) * CT_LD + 8 * t + lr];
+            // a * b : re = ar br - ai bi ; im = ar bi + ai br
+            dmma(cre[t][0], cre[t][1], av.x, bv.x); dmma(cre[t][0], cre[t][1], nai, bv.y);
+            dmma(cim[t][0], cim[t][1], av.x, bv.y); dmma(cim[t][0], cim[t][1], av.y, bv.x);
+          }
         }
       }
     }
+    __syncthreads();  // before the next tile refills the stages
     // epilogue: lambda^[k-1] on rows, lambda^[k+1] on columns, write into the stacked Jacobi matrix
     int rowoff = 0, coloff = 0;
     for (int ii = 0; ii < i; ++ii) rowoff += nbL[c + ii];
@@ -100,19 +124,23 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P
     const bool tr = rows < cols;
     const int ld = rows + cols;  // m + n
     cplx* Wd = P.W + P.goff[e];
+    const int a = a0 + 8 * warp + lr;
+    if (a < nL) {
+      const double la = lamL[a];
 #pragma unroll
-    for (int aa = 0; aa < 2; ++aa)
+      for (int t = 0; t < 4; ++t)
 #pragma unroll
-      for (int bb = 0; bb < 2; ++bb) {
-        const int a = a0 + ty * 2 + aa, b = b0 + tx * 2 + bb;
-        if (a < nL && b < nR) {
-          const double sc = lamL[a] * lamR[b];
-          cplx v = make_double2(acc[aa][bb].x * sc, acc[aa][bb].y * sc);
-          const long long r = rowoff + a, q = coloff + b;
-          if (!tr) Wd[r + q * ld] = v;
-          else Wd[q + r * ld] = make_double2(v.x, -v.y);
+        for (int x = 0; x < 2; ++x) {
+          const int b = b0 + 8 * t + 2 * lk + x;
+          if (b < nR) {
+            const double sc = la * lamR[b];
+            const cplx v = make_double2(cre[t][x] * sc, cim[t][x] * sc);
+            const long long r = rowoff + a, q = coloff + b;
+            if (!tr) Wd[r + q * ld] = v;
+            else Wd[q + r * ld] = make_double2(v.x, -v.y);
+          }
         }
-      }
+    }
   }
 }
 
@@ -133,7 +161,7 @@ __global__ void identity_kernel(Plan P) {
 
 void u1_launch_contract(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
   L.prof->begin(U1_ST_CONTRACT, L.stream);
-  contract_kernel<<<L.sms * 4, CT_THREADS, 0, L.stream>>>(S, P, G);
+  contract_kernel<<<L.sms * 8, CT_THREADS, 0, L.stream>>>(S, P, G);
   L.prof->end(L.stream);
   L.prof->begin(U1_ST_IDENTITY, L.stream);
   identity_kernel<<<L.sms * 2, 256, 0, L.stream>>>(P);
