@@ -31,6 +31,7 @@ namespace cg = cooperative_groups;
 #define SV_HLD 33                    // leading dimension of the 32 x 32 Gram matrix (row-major)
 #define SV_QLD 36                    // leading dimension of the transposed eigenvector matrix Qt (4 mod 8: B fragments)
 #define SV_INNER_MAX 2               // inner EVD sweeps per item (the outer iteration finishes the job; measured best of 1..4)
+#define SV_LASTPASS 1e-18            // (relative off-diagonal)^2 below which a rotation needs no verification sweep
 #define SV_QUAD 1e-14                // stop the inner EVD after a sweep whose largest relative off-diagonal^2 was below this
 #define SV_GROUP 128                 // threads per pair item; a CTA runs U1_SVD_THREADS / SV_GROUP = 4 items in lock-stepped phases
 #define SV_NGROUP (U1_SVD_THREADS / SV_GROUP)
@@ -457,7 +458,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
           const double tol = 8.0 * 1.1102230246251565e-16 * sqrt((double)I.m);
           I.tol2 = tol * tol;
         }
-        int todo = 0;
+        int todo = 0, big = 0;
         if (have) {
           gram_phase(stages, Hs, I, g, gtid);
           // quick test, same entries and arithmetic as the rotations: anything to do?
@@ -467,11 +468,17 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
               const double a = Hs[p * SV_HLD + p].x, b = Hs[qq * SV_HLD + qq].x;
               const cplx gg = Hs[p * SV_HLD + qq];
               const double ab = a * b, g2 = gg.x * gg.x + gg.y * gg.y;
-              todo |= (ab > 0.0 && g2 > I.tol2 * ab && g2 > 1e-290) ? 1 : 0;
+              if (ab > 0.0 && g2 > 1e-290) {
+                todo |= (g2 > I.tol2 * ab) ? 1 : 0;
+                big |= (g2 > SV_LASTPASS * ab) ? 1 : 0;
+              }
             }
           }
           todo = gsync_or(g, todo);
-          if (todo && gtid == 0) P.flags[e * U1_MAXSWEEP + sweep] = 1;
+          big = gsync_or(g, big);
+          // the sector needs another sweep only if some pivot was outside the quadratic regime: below it, this
+          // sweep's rotations leave relative off-diagonals of order 1e-6 sqrt(SV_LASTPASS) + SV_LASTPASS << tol
+          if (big && gtid == 0) P.flags[e * U1_MAXSWEEP + sweep] = 1;
         }
         __syncthreads();
         int inner = 0;
