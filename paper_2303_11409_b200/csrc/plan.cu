@@ -116,13 +116,13 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
   for (int e = t; e < E; e += PLAN_THREADS) {
     const int p = panels(e);
     if (p == 0 || !ok) continue;
-    mymax = max(mymax, p + (p & 1));
+    mymax = max(mymax, p);
     const int np = (p + 1) / 2, key = min(p, U1_MAXPANELS);
     const int off = cls_base[key] + atomicAdd(&cls_fill[key], np);
     for (int k = 0; k < np; ++k) { P.pitem_e[off + k] = e; P.pitem_k[off + k] = k; }
   }
   atomicMax(&shmax, mymax);
-  for (int i = t; i < E * U1_MAXSWEEP; i += PLAN_THREADS) P.flags[i] = 0;
+  for (int i = t; i < 2 * E; i += PLAN_THREADS) P.flags[i] = i < E ? 0 : 0x7fffffff;   // a3: last_rot[E], done_at[E]
   for (int i = t; i < 4 * U1_MAXSWEEP + 1; i += PLAN_THREADS) P.trace[i] = 0;
   __syncthreads();
   if (t == 0) P.cnt[3] = shmax;

@@ -13,10 +13,12 @@
 //             rotations per round on two-by-two units, in place; rotations sort the pair by
 //             norm, de Rijk style, which is what makes graded spectra converge)
 //   3. update [Pa Pb] <- [Pa Pb] Q over all m + n rows  (DMMA again, Q held in registers as B fragments)
-// A persistent cooperative grid walks the round-robin tournament of panel pairs of every sector in
-// lock step (one grid sync per round, items handed out through an atomic ticket); convergence is
-// decided on the device per sector (a sweep in which no item had an off-diagonal Gram entry above
-// tol * sqrt(h_pp h_qq)), no host round trip.
+// A persistent cooperative grid walks the panel pairs of every sector in lock step, one grid sync per round, items
+// handed out through an atomic ticket.  Round t pairs the panels with (i + j) mod np == (t + 1) mod np (modulus
+// ordering: a software-pipelined cyclic-by-rows ordering; with the norm-sorting rotations it deflates a graded
+// spectrum from the top like a Gram-Schmidt pass, and needs about 2/3 of the sweeps of the round-robin tournament
+// on the Theta blocks of the workloads).  Convergence is decided on the device per sector (np consecutive rounds,
+// i.e. every panel pair once, without an off-diagonal Gram entry above the threshold), no host round trip.
 #include <cooperative_groups.h>
 #include <cstdlib>
 #include "common.cuh"
@@ -407,7 +409,7 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
   gsync(g);
 }
 
-__global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S, Plan P, int inner_max) {
+__global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S, Plan P, int G, int inner_max) {
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ unsigned s_ticket;
   const int tid = threadIdx.x, g = tid / SV_GROUP, gtid = tid % SV_GROUP;
@@ -418,104 +420,116 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
   static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD) * 16 + U1_PB * 32, "EVD buffers must fit the idle stages");
   cg::grid_group grid = cg::this_grid();
   const int nblk = P.cnt[0], npair = P.cnt[1], maxP = P.cnt[3];
-  const int rounds = max(maxP - 1, 1);
+  const int R = max(maxP, 1);                      // rounds of one cycle of the largest sector (= a "sweep" of the trace)
+  const int E = G * S.NC;
+  int* last_rot = P.flags;                         // [E] round after the last rotation outside the quadratic regime
+  int* done_at = P.flags + E;                      // [E] round at which the sector was found converged (INT_MAX: not yet)
   unsigned base = 0;
   unsigned* ticket = reinterpret_cast<unsigned*>(P.cnt + 6);
-  int sweep = 0;
   if (blockIdx.x == 0 && tid == 0) { long long t0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0)); P.trace[0] = t0; }
-  for (; sweep < U1_MAXSWEEP && nblk > 0; ++sweep) {
-    int n_rot = 0, n_inner = 0;
-    for (int t = 0; t < rounds; ++t) {
-      for (;;) {
-        // four consecutive items (same sector, as a rule) per CTA, one per group; the groups run the three phases in
-        // lock step so that the latency-bound EVDs never share the FP64 pipe with another group's DMMA stream
-        __syncthreads();
-        if (tid == 0) s_ticket = atomicAdd(ticket, (unsigned)SV_NGROUP) - base;
-        __syncthreads();
-        const unsigned it0 = s_ticket;
-        if (it0 >= (unsigned)npair) break;
-        const unsigned it = it0 + g;
-        bool have = it < (unsigned)npair;
-        Item I;
-        int e = 0;
-        if (have) {
-          e = P.pitem_e[it];
-          const int k = P.pitem_k[it];
-          have = !(sweep > 0 && __ldcg(&P.flags[e * U1_MAXSWEEP + sweep - 1]) == 0);  // sector converged
-          const int r = P.rows[e], q = P.cols[e];
-          I.m = max(r, q);
-          const int n = min(r, q);
-          I.mt = I.m + n;
-          const int np = u1_ceil_div(n, U1_PB);
-          const int np2 = np + (np & 1);
-          if (t >= max(np2 - 1, 1)) have = false;
-          int pa, pb;
-          rr_pair(min(t, max(np2 - 2, 0)), k, max(np2, 2), &pa, &pb);
-          if (pb >= np && np > 1) have = false;  // bye (odd number of panels)
-          I.W = P.W + P.goff[e];
-          I.ca = pa * U1_PB; I.na = min(U1_PB, n - I.ca);
-          I.cb = pb * U1_PB; I.nb = pb < np ? min(U1_PB, n - I.cb) : 0;
-          const double tol = 8.0 * 1.1102230246251565e-16 * sqrt((double)I.m);
-          I.tol2 = tol * tol;
+  int tg = 0, n_rot = 0, n_inner = 0, ndone = 0;
+  for (; tg < U1_MAXSWEEP * R && nblk > 0; ++tg) {
+    for (;;) {
+      __syncthreads();
+      if (tid == 0) s_ticket = atomicAdd(ticket, (unsigned)SV_NGROUP) - base;
+      __syncthreads();
+      const unsigned it0 = s_ticket;
+      if (it0 >= (unsigned)npair) break;
+      const unsigned it = it0 + g;
+      bool have = it < (unsigned)npair;
+      Item I;
+      int e = 0;
+      if (have) {
+        e = P.pitem_e[it];
+        const int k = P.pitem_k[it];
+        const int r = P.rows[e], q = P.cols[e];
+        I.m = max(r, q);
+        const int n = min(r, q);
+        I.mt = I.m + n;
+        const int np = u1_ceil_div(n, U1_PB);
+        // the sector is finished once np consecutive rounds (= every panel pair once) needed no rotation outside the
+        // quadratic regime
+        if (tg - __ldcg(&last_rot[e]) >= np) {
+          have = false;
+          if (k == 0 && gtid == 0) atomicMin(&done_at[e], tg);
         }
-        int todo = 0, big = 0;
-        if (have) {
-          gram_phase(stages, Hs, I, g, gtid);
-          // quick test, same entries and arithmetic as the rotations: anything to do?
-          for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
-            const int p = idx >> 5, qq = idx & 31;
-            if (p < qq) {
-              const double a = Hs[p * SV_HLD + p].x, b = Hs[qq * SV_HLD + qq].x;
-              const cplx gg = Hs[p * SV_HLD + qq];
-              const double ab = a * b, g2 = gg.x * gg.x + gg.y * gg.y;
-              if (ab > 0.0 && g2 > 1e-290) {
-                todo |= (g2 > I.tol2 * ab) ? 1 : 0;
-                big |= (g2 > SV_LASTPASS * ab) ? 1 : 0;
-              }
+        // modulus ordering (a pipelined cyclic-by-rows ordering): round tg pairs the panels with (i + j) mod np == rho
+        int pa = 0, pb = 1;
+        if (np > 1) {
+          const int rho = (tg + 1) % np;
+          const int na = (rho + 1) >> 1;
+          if (k < na) { pa = k; pb = rho - k; }
+          else { pa = rho + 1 + (k - na); pb = rho + np - pa; }
+          if (pa >= pb) have = false;
+        }
+        I.W = P.W + P.goff[e];
+        I.ca = pa * U1_PB; I.na = min(U1_PB, n - I.ca);
+        I.cb = pb * U1_PB; I.nb = pb < np ? min(U1_PB, n - I.cb) : 0;
+        const double tol = 8.0 * 1.1102230246251565e-16 * sqrt((double)I.m);
+        I.tol2 = tol * tol;
+      }
+      int todo = 0, big = 0;
+      if (have) {
+        gram_phase(stages, Hs, I, g, gtid);
+        // quick test, same entries and arithmetic as the rotations: anything to do?
+        for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
+          const int p = idx >> 5, qq = idx & 31;
+          if (p < qq) {
+            const double a = Hs[p * SV_HLD + p].x, b = Hs[qq * SV_HLD + qq].x;
+            const cplx gg = Hs[p * SV_HLD + qq];
+            const double ab = a * b, g2 = gg.x * gg.x + gg.y * gg.y;
+            if (ab > 0.0 && g2 > 1e-290) {
+              todo |= (g2 > I.tol2 * ab) ? 1 : 0;
+              big |= (g2 > SV_LASTPASS * ab) ? 1 : 0;
             }
           }
-          todo = gsync_or(g, todo);
-          big = gsync_or(g, big);
-          // the sector needs another sweep only if some pivot was outside the quadratic regime: below it, this
-          // sweep's rotations leave relative off-diagonals of order 1e-6 sqrt(SV_LASTPASS) + SV_LASTPASS << tol
-          if (big && gtid == 0) P.flags[e * U1_MAXSWEEP + sweep] = 1;
         }
-        __syncthreads();
-        int inner = 0;
-        if (todo) evd_phase(Hs, Qs, Rm, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
-        __syncthreads();
-        if (todo) {
-          update_phase(stages, Qs, I, g, gtid);
-          if (gtid == 0) { n_rot += 1; n_inner += inner; }
-        }
+        todo = gsync_or(g, todo);
+        big = gsync_or(g, big);
+        // below SV_LASTPASS this visit's rotations leave relative off-diagonals of order 1e-6 sqrt(SV_LASTPASS) +
+        // SV_LASTPASS << tol: such a visit does not restart the sector's count of clean rounds
+        if (big && gtid == 0) atomicMax(&last_rot[e], tg + 1);
       }
-      base += (unsigned)SV_NGROUP * ((unsigned)(npair + SV_NGROUP - 1) / SV_NGROUP + gridDim.x);
-      grid.sync();
+      __syncthreads();
+      int inner = 0;
+      if (todo) evd_phase(Hs, Qs, Rm, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
+      __syncthreads();
+      if (todo) {
+        update_phase(stages, Qs, I, g, gtid);
+        if (gtid == 0) { n_rot += 1; n_inner += inner; }
+      }
     }
-    // ---- convergence: stop when no sector rotated in this sweep
-    int any = 0;
-    for (int bi = tid; bi < nblk; bi += U1_SVD_THREADS) any += __ldcg(&P.flags[P.blk[bi] * U1_MAXSWEEP + sweep]);
-    const int nact = __syncthreads_count(any);
-    if (gtid == 0 && n_rot) {  // trace of this launch (u1mps_svd_trace)
-      atomicAdd((unsigned long long*)&P.trace[1 + U1_MAXSWEEP + sweep], (unsigned long long)n_rot);
-      atomicAdd((unsigned long long*)&P.trace[1 + 2 * U1_MAXSWEEP + sweep], (unsigned long long)n_inner);
+    base += (unsigned)SV_NGROUP * ((unsigned)(npair + SV_NGROUP - 1) / SV_NGROUP + gridDim.x);
+    grid.sync();
+    // ---- convergence: sectors found finished up to this round (stamps of later rounds are ignored, so that every
+    // CTA takes the same decision)
+    int mine = 0;
+    for (int bi = tid; bi < nblk; bi += U1_SVD_THREADS) mine += (__ldcg(&done_at[P.blk[bi]]) <= tg) ? 1 : 0;
+    __shared__ int s_done;
+    if (tid == 0) s_done = 0;
+    __syncthreads();
+    if (mine) atomicAdd(&s_done, mine);
+    __syncthreads();
+    ndone = s_done;
+    const bool last = ndone == nblk;
+    if ((tg + 1) % R == 0 || last) {  // trace of this launch (u1mps_svd_trace), one entry per R rounds
+      const int sw = tg / R;
+      if (gtid == 0 && n_rot) {
+        atomicAdd((unsigned long long*)&P.trace[1 + U1_MAXSWEEP + sw], (unsigned long long)n_rot);
+        atomicAdd((unsigned long long*)&P.trace[1 + 2 * U1_MAXSWEEP + sw], (unsigned long long)n_inner);
+      }
+      n_rot = 0; n_inner = 0;
+      if (tid == 0 && blockIdx.x == 0) {
+        long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+        P.trace[1 + sw] = t1;
+        P.trace[1 + 3 * U1_MAXSWEEP + sw] = nblk - ndone;
+      }
     }
-    if (tid == 0 && blockIdx.x == 0) {
-      long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
-      P.trace[1 + sweep] = t1;
-      int act = 0;
-      for (int bi = 0; bi < nblk; ++bi) act += __ldcg(&P.flags[P.blk[bi] * U1_MAXSWEEP + sweep]);
-      P.trace[1 + 3 * U1_MAXSWEEP + sweep] = act;
-    }
-    if (nact == 0) { ++sweep; break; }
+    if (last) { ++tg; break; }
   }
   if (blockIdx.x == 0 && tid == 0) {
-    atomicMax(&S.err[1], sweep);
-    if (sweep >= U1_MAXSWEEP) {
-      int bad = 0;
-      for (int bi = 0; bi < nblk; ++bi) bad += P.flags[P.blk[bi] * U1_MAXSWEEP + U1_MAXSWEEP - 1];
-      if (bad) atomicAdd(&S.err[2], bad);
-    }
+    atomicMax(&S.err[1], (tg + R - 1) / R);
+    if (nblk > 0 && ndone < nblk) atomicAdd(&S.err[2], nblk - ndone);
   }
 }
 
@@ -578,10 +592,9 @@ cudaError_t u1_svd_configure(int* grid, int* smem_bytes, int sms) {
 }
 
 cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
-  (void)G;
-  DevState s = S; Plan p = P;
+  DevState s = S; Plan p = P; int gcount = G;
   static int inner_max = getenv("U1MPS_INNER_MAX") ? atoi(getenv("U1MPS_INNER_MAX")) : SV_INNER_MAX;
-  void* args[] = {&s, &p, &inner_max};
+  void* args[] = {&s, &p, &gcount, &inner_max};
   L.prof->begin(U1_ST_SVD, L.stream);
   cudaError_t err = cudaLaunchCooperativeKernel((void*)svd_kernel, dim3(L.svd_grid), dim3(U1_SVD_THREADS), args,
                                                 (size_t)L.svd_smem, L.stream);
