@@ -214,7 +214,8 @@ __device__ __forceinline__ double rcp_approx(double x) { double y; asm("rcp.appr
 // Work split of a round: thread k < hp computes rotation k and rewrites its own 2 x 2 pivot block (closed form);
 // after the barrier every 2 x 2 unit (rows of pivot ki, columns of pivot kj, ki < kj) is read, rotated from both
 // sides and written, together with its mirror image, by one thread (H stays exactly Hermitian); the Q units
-// (two rows x the two columns of a pivot) likewise.  Pivot indices advance by one (mod 2hp - 1) per round.
+// (two rows x the two columns of a pivot) likewise.  The pivots of a round come from a small shared-memory table of the
+// modulus ordering (pairs with (i + j) mod 2hp == round), the same pipelined cyclic-by-rows ordering as the outer one.
 struct Rot { double cs, sr, si; int flag; };   // flag: 0 idle, 1 rotate, 3 rotate and exchange
 __device__ __forceinline__ Rot load_rot(const double4* Rm, int k) {
   const double4 v = Rm[k];
@@ -233,14 +234,23 @@ __device__ __forceinline__ void rot_rows(cplx& x, cplx& y, const Rot& r) {
   const cplx yn = make_double2(fma(r.sr, x.x, fma(r.si, x.y, r.cs * y.x)), fma(r.sr, x.y, fma(-r.si, x.x, r.cs * y.y)));
   x = xn; y = yn;
 }
-__device__ __forceinline__ void advance(int& p, int& q, int k, int m) {  // pivot k of the next round
-  if (++p == m) p = 0;
-  if (k != 0 && ++q == m) q = 0;
+// Pivot k of the round with residue rho of the modulus ordering over n players (n even, n/2 slots): the pairs
+// (i, j), i < j, with (i + j) mod n == rho.  For even rho two players stay unpaired: they fill the last slot as an
+// idle pivot (returned with bit 7 of q set), so that every row and column of H belongs to exactly one slot.
+__device__ __forceinline__ uchar2 mod_pivot(int rho, int k, int n) {
+  const int na = (rho + 1) >> 1;                       // pairs with i + j == rho
+  const int nb = max(((rho + n + 1) >> 1) - rho - 1, 0);  // pairs with i + j == rho + n
+  int p, q;
+  if (k < na) { p = k; q = rho - k; }
+  else if (k - na < nb) { p = rho + 1 + (k - na); q = rho + n - p; }
+  else { p = rho >> 1; q = ((rho + n) >> 1) | 0x80; }
+  return make_uchar2((unsigned char)p, (unsigned char)q);
 }
 
-__device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, int hp, double tol2, int* inner, int inner_max, int g, int gtid) {
+__device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2* tab, int hp, double tol2, int* inner, int inner_max, int g, int gtid) {
   const int tid = gtid;
-  const int np2 = 2 * hp, m = np2 - 1;
+  const int np2 = 2 * hp;
+  for (int idx = tid; idx < np2 * hp; idx += SV_GROUP) tab[idx] = mod_pivot(idx / hp, idx % hp, np2);
   for (int idx = tid; idx < SV_W * SV_QLD; idx += SV_GROUP) {
     const int c = idx / SV_QLD, r = idx - c * SV_QLD;
     Qt[idx] = make_double2(r == c ? 1.0 : 0.0, 0.0);
@@ -261,19 +271,17 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, int hp
   for (int sw = 0; sw < inner_max; ++sw) {
     double mymax = 0.0;
     int sweep_any = 0;
-    // pivots at round 0: (k, m - k) for k >= 1, (0, m) for k = 0
-    int pp = tid < hp ? tid : 0, pq = tid < hp ? m - tid : 0;                 // rotation owned by this thread (tid < hp)
-    int pi = max(uki, 0), qi = m - max(uki, 0), pj = ukj, qj = m - ukj;         // H unit
-    int pc0 = kq0, qc0 = m - kq0, pc1 = kq0 + 8, qc1 = m - kq0 - 8;            // Q units
-    for (int t = 0; t < m; ++t) {
+    for (int t = 0; t < np2; ++t) {
+      const uchar2* row = tab + ((t + 1) % np2) * hp;   // pivots of this round
       int rot = 0;
       if (tid < hp) {
-        const int p = pp, q = pq;
+        const uchar2 pv = row[tid];
+        const int p = pv.x, q = pv.y & 0x7f;
         const double a = H[p * SV_HLD + p].x, b = H[q * SV_HLD + q].x;
         const cplx gg = H[p * SV_HLD + q];
         const double g2 = gg.x * gg.x + gg.y * gg.y, ab = a * b;
         double4 out = make_double4(1.0, 0.0, 0.0, 0.0);
-        if (ab > 0.0 && g2 > tol2 * ab && g2 > 1e-290) {
+        if (!(pv.y & 0x80) && ab > 0.0 && g2 > tol2 * ab && g2 > 1e-290) {
           rot = 1;
           mymax = fmax(mymax, g2 * rcp_approx(ab));
           const double iag = rsqrt_approx(g2);                 // ~ 1/|g|
@@ -314,6 +322,8 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, int hp
         if (uki >= 0) {
           const Rot ri = load_rot(Rm, uki), rj = load_rot(Rm, ukj);
           if (ri.flag | rj.flag) {
+            const uchar2 vi = row[uki], vj = row[ukj];
+            const int pi = vi.x, qi = vi.y & 0x7f, pj = vj.x, qj = vj.y & 0x7f;
             cplx b00 = H[pi * SV_HLD + pj], b01 = H[pi * SV_HLD + qj], b10 = H[qi * SV_HLD + pj], b11 = H[qi * SV_HLD + qj];
             if (rj.flag) { rot_cols(b00, b01, rj); rot_cols(b10, b11, rj); }
             if (ri.flag) { rot_rows(b00, b10, ri); rot_rows(b01, b11, ri); }
@@ -330,7 +340,8 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, int hp
           if (x < nq) {
             const Rot rj = load_rot(Rm, kq0 + 8 * x);
             if (rj.flag) {
-              const int pc = x ? pc1 : pc0, qc = x ? qc1 : qc0;
+              const uchar2 vc = row[kq0 + 8 * x];
+              const int pc = vc.x, qc = vc.y & 0x7f;
               cplx* cp = Qt + pc * SV_QLD + rp;
               cplx* cq = Qt + qc * SV_QLD + rp;
               cplx q00 = cp[0], q01 = cq[0], q10 = cp[hp], q11 = cq[hp];
@@ -343,9 +354,6 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, int hp
         }
         gsync(g);
       }
-      advance(pp, pq, tid, m);
-      advance(pi, qi, uki, m); advance(pj, qj, ukj, m);
-      advance(pc0, qc0, kq0, m); advance(pc1, qc1, kq0 + 8, m);
     }
     if (!sweep_any) break;
     ++*inner;
@@ -417,7 +425,8 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
   cplx* Hs = stages;                               // [32*33], aliased onto the ring (idle during the EVD)
   cplx* Qs = Hs + SV_W * SV_HLD;                   // [32*36], transposed
   double4* Rm = reinterpret_cast<double4*>(Qs + SV_W * SV_QLD);   // [16] rotations of the current EVD round
-  static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD) * 16 + U1_PB * 32, "EVD buffers must fit the idle stages");
+  uchar2* tab = reinterpret_cast<uchar2*>(Rm + U1_PB);             // [32][16] pivots of the modulus ordering
+  static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD) * 16 + U1_PB * 32 + SV_W * U1_PB * 2, "EVD buffers must fit the idle stages");
   cg::grid_group grid = cg::this_grid();
   const int nblk = P.cnt[0], npair = P.cnt[1], maxP = P.cnt[3];
   const int R = max(maxP, 1);                      // rounds of one cycle of the largest sector (= a "sweep" of the trace)
@@ -492,7 +501,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
       }
       __syncthreads();
       int inner = 0;
-      if (todo) evd_phase(Hs, Qs, Rm, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
+      if (todo) evd_phase(Hs, Qs, Rm, tab, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
       __syncthreads();
       if (todo) {
         update_phase(stages, Qs, I, g, gtid);
