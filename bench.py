@@ -404,7 +404,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=3, help="BASELINE.json config index (1-based); 3 = chi=1024")
     ap.add_argument("--prep-columns", type=int, default=-1, help="columns run before timing (-1: the config's own)")
-    ap.add_argument("--cpu-gates", type=int, default=24, help="oracle gates in the cpu_baseline sample")
+    ap.add_argument("--cpu-gates", type=int, default=96, help="oracle gates in the cpu_baseline sample")
     ap.add_argument("--ref-gates", type=int, default=8, help="oracle gates per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -9,9 +9,8 @@
 // (32 columns):
 //   1. Gram   H = P^H P over the m rows of G           (FP64 DMMA.8x8x4 tiles, chunks of 32 rows staged
 //                                                        in shared memory by a 2-stage cp.async ring)
-//   2. EVD    H = Q diag Q^H by two-sided Jacobi in shared memory (parallel round-robin ordering, 16
-//             rotations per round on two-by-two units, in place; rotations sort the pair by
-//             norm, de Rijk style, which is what makes graded spectra converge)
+//   2. EVD    H = Q diag Q^H by two-sided Jacobi in shared memory (16 disjoint rotations per round on
+//             two-by-two units, in place; rotations sort the pair by norm, de Rijk style)
 //   3. update [Pa Pb] <- [Pa Pb] Q over all m + n rows  (DMMA again, Q held in registers as B fragments)
 // A persistent cooperative grid walks the panel pairs of every sector in lock step, one grid sync per round, items
 // handed out through an atomic ticket.  Round t pairs the panels with (i + j) mod np == (t + 1) mod np (modulus
@@ -35,10 +34,10 @@ namespace cg = cooperative_groups;
 #define SV_INNER_MAX 2               // inner EVD sweeps per item (the outer iteration finishes the job; measured best of 1..4)
 #define SV_LASTPASS 1e-18            // (relative off-diagonal)^2 below which a rotation needs no verification sweep
 #define SV_QUAD 1e-14                // stop the inner EVD after a sweep whose largest relative off-diagonal^2 was below this
-#define SV_GROUP 128                 // threads per pair item; a CTA runs U1_SVD_THREADS / SV_GROUP = 4 items in lock-stepped phases
+#define SV_GROUP 128                 // threads per pair item (= one CTA: SV_NGROUP == 1; several groups per CTA were tried and dropped)
 #define SV_NGROUP (U1_SVD_THREADS / SV_GROUP)
 #define SV_CTAS 6                    // resident CTAs per SM the kernel is compiled for (registers <= 85)
-#define SV_GROUP_BYTES (SV_NSTAGE * SV_STAGE * 16)   // 55,296 B per group
+#define SV_GROUP_BYTES (SV_NSTAGE * SV_STAGE * 16)   // 36,864 B per group
 #define SV_SMEM_BYTES (SV_NGROUP * SV_GROUP_BYTES)
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -61,7 +60,7 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
-// Named barriers of a 128-thread group (ids 1..4; 0 is __syncthreads) and its block-wide OR.
+// Named barrier of a 128-thread group (id g + 1; 0 is __syncthreads) and its group-wide OR.
 __device__ __forceinline__ void gsync(int g) { asm volatile("bar.sync %0, 128;\n" ::"r"(g + 1) : "memory"); }
 __device__ __forceinline__ int gsync_or(int g, int pred) {
   int r;
@@ -77,24 +76,10 @@ __device__ __forceinline__ cplx cmulc(cplx a, cplx b) {  // conj(a) * b
 __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
 // a b + c d  and  conj(a) b + conj(c) d, as fused chains (8 FP64 instructions each)
 __device__ __forceinline__ cplx cdot2(cplx a, cplx b, cplx c, cplx d) {
-#ifdef U1_SLOWCPLX
-  return cadd(cmul(a, b), cmul(c, d));
-#endif
   return make_double2(fma(a.x, b.x, fma(-a.y, b.y, fma(c.x, d.x, -c.y * d.y))), fma(a.x, b.y, fma(a.y, b.x, fma(c.x, d.y, c.y * d.x))));
 }
 __device__ __forceinline__ cplx cdot2c(cplx a, cplx b, cplx c, cplx d) {
-#ifdef U1_SLOWCPLX
-  return cadd(cmulc(a, b), cmulc(c, d));
-#endif
   return make_double2(fma(a.x, b.x, fma(a.y, b.y, fma(c.x, d.x, c.y * d.y))), fma(a.x, b.y, fma(-a.y, b.x, fma(c.x, d.y, -c.y * d.x))));
-}
-
-// circle-method round robin over np2 (even) players: slot k of round t -> (a, b), a < b
-__device__ __forceinline__ void rr_pair(int t, int k, int np2, int* a, int* b) {
-  const int q = np2 - 1;
-  if (k == 0) { *a = t % q; *b = q; }
-  else { *a = (t + k) % q; *b = (t - k + 2 * q) % q; }
-  if (*a > *b) { int s = *a; *a = *b; *b = s; }
 }
 
 struct Item {
