@@ -301,15 +301,21 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
         }
         Rm[tid] = out;
       }
+      // this thread's H unit is loaded while warp 0 works out the rotations (the rotation threads only rewrite their
+      // own pivot blocks, never an off-diagonal unit)
+      int pi = 0, qi = 0, pj = 0, qj = 0;
+      cplx b00, b01, b10, b11;
+      if (uki >= 0) {
+        const uchar2 vi = row[uki], vj = row[ukj];
+        pi = vi.x; qi = vi.y & 0x7f; pj = vj.x; qj = vj.y & 0x7f;
+        b00 = H[pi * SV_HLD + pj]; b01 = H[pi * SV_HLD + qj]; b10 = H[qi * SV_HLD + pj]; b11 = H[qi * SV_HLD + qj];
+      }
       const int any = gsync_or(g, rot);
       if (any) {  // uniform
         sweep_any = 1;
         if (uki >= 0) {
           const Rot ri = load_rot(Rm, uki), rj = load_rot(Rm, ukj);
           if (ri.flag | rj.flag) {
-            const uchar2 vi = row[uki], vj = row[ukj];
-            const int pi = vi.x, qi = vi.y & 0x7f, pj = vj.x, qj = vj.y & 0x7f;
-            cplx b00 = H[pi * SV_HLD + pj], b01 = H[pi * SV_HLD + qj], b10 = H[qi * SV_HLD + pj], b11 = H[qi * SV_HLD + qj];
             if (rj.flag) { rot_cols(b00, b01, rj); rot_cols(b10, b11, rj); }
             if (ri.flag) { rot_rows(b00, b10, ri); rot_rows(b01, b11, ri); }
             // exchanges are applied to the destinations
@@ -587,6 +593,7 @@ cudaError_t u1_svd_configure(int* grid, int* smem_bytes, int sms) {
 
 cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
   DevState s = S; Plan p = P; int gcount = G;
+  // tuning knob for experiments only: inner EVD sweeps per item, default SV_INNER_MAX
   static int inner_max = getenv("U1MPS_INNER_MAX") ? atoi(getenv("U1MPS_INNER_MAX")) : SV_INNER_MAX;
   void* args[] = {&s, &p, &gcount, &inner_max};
   L.prof->begin(U1_ST_SVD, L.stream);

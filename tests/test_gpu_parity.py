@@ -96,19 +96,32 @@ def test_teacher_forced_every_gate(idx, M, N, chi, cols):
 
 
 # ------------------------------------------------------------------ synthetic saturated bonds: several tiles, ragged tails,
-# all three Jacobi paths (two panels in smem with b=16, b=8, and in place through L2)
+# single- and multi-panel sectors, several 32-row chunks, ragged panel and chunk tails
 @pytest.mark.parametrize("d,chi,R,keep_chi", [
-    (2, 96, 4, 64),       # sectors ~ 24..48 wide: single/multi panel, b = 16
-    (2, 333, 5, 200),     # ragged: blocks ~ 130 x 150, m + n <= 400 -> b = 16 in smem
-    (2, 700, 4, 512),     # m + n ~ 700 -> b = 8 in smem
-    (2, 1024, 3, 1024),   # m + n > 800 -> in-place path
+    (2, 96, 4, 64),       # sectors ~ 24..48 wide: 2-4 panels
+    (2, 333, 5, 200),     # ragged: blocks ~ 130 x 150
+    (2, 700, 4, 512),     # blocks ~ 350 x 350
+    (2, 1024, 3, 1024),   # blocks ~ 680 x 680 (43 panels)
     (4, 256, 6, 256),     # d = 4: rows(c) spans 4 left sectors
     (5, 180, 7, 100),     # d = 5
 ])
 def test_synthetic_gate(d, chi, R, keep_chi):
-    M, N, s, lam, gam = inputs.synthetic_gate_state(d, chi, R, seed=1234 + chi)
+    _synthetic_case(d, chi, R, keep_chi)
+
+
+def test_saturated_profile_chi1024_xxz_gate():
+    """Full-size parity case of the bench workload: the sector sizes measured on config 3's saturated bonds
+    (Theta(c) blocks up to 485 x 485, 31 panels: every phase of the block Jacobi at the size bench.py times),
+    the config's own XXZ gate, truncation back to chi = 1024."""
+    w = inputs.WORKLOADS[3]
+    _synthetic_case(2, 1024, 10, 1024, profile=inputs.SATURATED_PROFILE[3], U=inputs.xxz_gate(w.delta, w.dt))
+
+
+def _synthetic_case(d, chi, R, keep_chi, profile=None, U=None):
+    M, N, s, lam, gam = inputs.synthetic_gate_state(d, chi, R, seed=1234 + chi, profile=profile)
     rng = np.random.default_rng(99 + chi)
-    U = inputs.random_u1_gate(rng, d, unitary=(d == 2))
+    if U is None:
+        U = inputs.random_u1_gate(rng, d, unitary=(d == 2))
     occ = [0] * M
     left = N
     for i in range(M):
@@ -233,3 +246,32 @@ def test_error_codes():
         gpu.apply_gate_column([0, 1], np.stack([np.eye(4, dtype=np.complex128)] * 2))   # overlapping gates
     assert e.value.code == -1
     assert np.allclose(gpu.expect_n_all(), [1, 0, 1, 0, 1, 0])
+
+
+def test_svd_trace_and_convergence_bookkeeping():
+    """u1mps_svd_trace: one entry per sweep of the last a3 launch; the last entry has no active sector left."""
+    d, chi, R = 2, 333, 5
+    M, N, s, lam, gam = inputs.synthetic_gate_state(d, chi, R, seed=77)
+    occ, left = [0] * M, N
+    for i in range(M):
+        occ[i] = min(d - 1, left)
+        left -= occ[i]
+    ora = Oracle.product_state(M, d, N, chi, occ)
+    for k in (2, 3, 4):
+        ora.sectors[k] = sorted(lam[k])
+        ora.lam[k] = lam[k]
+    for st in (2, 3):
+        ora.gam[st] = gam[st]
+    gpu = make_gpu(M, d, N, chi)
+    gpu.set_product_state(occ)
+    oracle_to_gpu(ora, gpu, bonds=[2, 3, 4], sites=[2, 3])
+    gpu.apply_two_site_gate(s, inputs.random_u1_gate(np.random.default_rng(3), d))
+    tr = gpu.svd_trace()
+    gpu.truncate(s, chi, 1e-12)
+    st = gpu.last_stats()
+    assert st["converged"]
+    n = len(tr["sweep_ms"])
+    assert n == st["sweeps"] and 2 <= n <= 30
+    assert np.all(tr["sweep_ms"] > 0)
+    assert tr["rotated_items"][0] > 0 and tr["inner_sweeps"][0] >= tr["rotated_items"][0]
+    assert tr["active_sectors"][-1] == 0 and np.all(np.diff(tr["active_sectors"]) <= 0)
