@@ -36,7 +36,7 @@ Sizes compute_sizes(int M, int d, int N, int chi) {
   z.Gmax = std::max(1, M / 2);
   const size_t E = (size_t)z.Gmax * NC;
   z.poolcap = (int)std::min<size_t>((size_t)z.Gmax * d * chi, (size_t)1 << 30);
-  z.itemcap = z.poolcap / (U1_PANEL / 2) + (int)E + 16;
+  z.itemcap = z.poolcap / (2 * U1_PB) + (int)E + 16;   // sum over entries of (ceil(n / U1_PB) + 1) / 2
   size_t b = 0;
   auto add = [&](size_t bytes) { b = ((b + 255) & ~(size_t)255) + bytes; };
   add((M + 1) * NC * 4); add((M + 1) * NC * 4);                  // nb, ob
@@ -48,7 +48,7 @@ Sizes compute_sizes(int M, int d, int N, int chi) {
   for (int i = 0; i < 5; ++i) add((E + 1) * 4);                  // rows cols keep blk tmpa
   add((E + 1) * 8); add((E + 1) * 4);                            // goff svoff
   add((E * d * d + 1) * 4); add((2 * E + 1) * 4);                // t2pref t5pref
-  add(8 * 4); add(E * U1_MAXSWEEP * 4); add((size_t)2 * z.Gmax * 8);  // cnt flags gate_w
+  add(8 * 4); add(2 * E * 4); add((size_t)2 * z.Gmax * 8);  // cnt flags gate_w
   add((4 * U1_MAXSWEEP + 1) * 8);                                // trace
   for (int i = 0; i < 2; ++i) add((size_t)z.itemcap * 4);        // item lists
   add((size_t)z.poolcap * 4); add((size_t)z.poolcap * 8); add((size_t)z.poolcap * 8);  // perm sv svs
@@ -210,7 +210,7 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
   P.blk = A.take<int>(E + 1); P.tmpa = A.take<int>(E + 1);
   P.goff = A.take<long long>(E + 1); P.svoff = A.take<int>(E + 1);
   P.t2pref = A.take<int>(E * d * d + 1); P.t5pref = A.take<int>(2 * E + 1);
-  P.cnt = A.take<int>(8); P.flags = A.take<int>(E * U1_MAXSWEEP); P.gate_w = A.take<double>((size_t)2 * z.Gmax);
+  P.cnt = A.take<int>(8); P.flags = A.take<int>(2 * E); P.gate_w = A.take<double>((size_t)2 * z.Gmax);
   P.trace = A.take<long long>(4 * U1_MAXSWEEP + 1);
   P.pitem_e = A.take<int>(z.itemcap); P.pitem_k = A.take<int>(z.itemcap);
   P.perm = A.take<int>(z.poolcap); P.sv = A.take<double>(z.poolcap); P.svs = A.take<double>(z.poolcap);
@@ -602,7 +602,7 @@ int u1mps_export_staged_svd(u1mps_t* h, int c, void* V, double* sigma, void* Wou
       for (int j = 0; j < n; ++j) {
         const int p = perm[j];
         cplx v = tr ? buf[(size_t)(p * ld + m + a)] : buf[(size_t)(p * ld + a)];
-        if (!tr) { v.x /= sv[j]; v.y /= sv[j]; }
+        if (!tr && sv[j] > 0.0) { v.x /= sv[j]; v.y /= sv[j]; }   // an exactly zero column stays zero
         o[(size_t)a * n + j] = v;
       }
   }
@@ -612,7 +612,7 @@ int u1mps_export_staged_svd(u1mps_t* h, int c, void* V, double* sigma, void* Wou
       for (int b = 0; b < cols; ++b) {
         const int p = perm[j];
         cplx v = tr ? buf[(size_t)(p * ld + b)] : buf[(size_t)(p * ld + m + b)];
-        if (tr) { v.x /= sv[j]; v.y /= sv[j]; }
+        if (tr && sv[j] > 0.0) { v.x /= sv[j]; v.y /= sv[j]; }
         v.y = -v.y;
         o[(size_t)j * cols + b] = v;
       }

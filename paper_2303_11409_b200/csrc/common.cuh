@@ -8,7 +8,6 @@ typedef double2 cplx;  // complex128, interleaved (x = re, y = im), 16-byte alig
 
 #define U1_TILE 32         // a2 / a5 tile edge
 #define U1_MAXSWEEP 30     // Jacobi (outer) sweep limit
-#define U1_PANEL 16        // (item-list sizing unit)
 #define U1_PB 16           // columns per Jacobi panel: a pair item orthogonalises 2*U1_PB = 32 columns
 #define U1_ERR_WORKSPACE 1 // device error flag: plan does not fit the workspace
 #define U1_SVD_THREADS 128 // 4 warps per pair item, 6 CTAs per SM
@@ -43,7 +42,7 @@ struct Plan {
   int* pitem_k;      // [cap] ... pair slot k of the round-robin tournament
   int* tmpa;         // [G*NC+1] scratch: pair-item offset per entry
   int* cnt;          // [8] 0: #blk, 1: #pair items, 3: max panels (even), 4: a2 tiles, 5: a5 tiles, 6: a3 work-queue ticket, 7: a4 CTA counter
-  int* flags;        // [G*NC*U1_MAXSWEEP] per entry, per sweep: 1 if any rotation happened
+  int* flags;        // [2*G*NC] a3 convergence stamps per entry: round after the last counting rotation, round found finished
   long long* trace;  // [4*U1_MAXSWEEP] a3 trace of the last launch: per sweep end time (globaltimer ns), rotated items, inner sweeps, active sectors
   int* keep;         // [G*NC] kept singular values per entry (a4)
   int* perm;         // [pool] sorted position -> column index

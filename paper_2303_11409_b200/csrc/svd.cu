@@ -30,6 +30,7 @@ namespace cg = cooperative_groups;
 #define SV_STAGE (SV_W * SV_LDG)     // complex elements per stage
 #define SV_NSTAGE 2
 #define SV_HLD 33                    // leading dimension of the 32 x 32 Gram matrix (row-major)
+static_assert(U1_MAXSWEEP == 30, "keep U1MPS_MAXSWEEP of include/u1mps.h in step");
 #define SV_QLD 36                    // leading dimension of the transposed eigenvector matrix Qt (4 mod 8: B fragments)
 #define SV_INNER_MAX 2               // inner EVD sweeps per item (the outer iteration finishes the job; measured best of 1..4)
 #define SV_LASTPASS 1e-18            // (relative off-diagonal)^2 below which a rotation needs no verification sweep
@@ -67,19 +68,6 @@ __device__ __forceinline__ int gsync_or(int g, int pred) {
   asm volatile("{\n .reg .pred p, q;\n setp.ne.s32 p, %2, 0;\n bar.red.or.pred q, %1, 128, p;\n selp.s32 %0, 1, 0, q;\n}\n"
                : "=r"(r) : "r"(g + 1), "r"(pred) : "memory");
   return r;
-}
-
-__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
-__device__ __forceinline__ cplx cmulc(cplx a, cplx b) {  // conj(a) * b
-  return make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
-}
-__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
-// a b + c d  and  conj(a) b + conj(c) d, as fused chains (8 FP64 instructions each)
-__device__ __forceinline__ cplx cdot2(cplx a, cplx b, cplx c, cplx d) {
-  return make_double2(fma(a.x, b.x, fma(-a.y, b.y, fma(c.x, d.x, -c.y * d.y))), fma(a.x, b.y, fma(a.y, b.x, fma(c.x, d.y, c.y * d.x))));
-}
-__device__ __forceinline__ cplx cdot2c(cplx a, cplx b, cplx c, cplx d) {
-  return make_double2(fma(a.x, b.x, fma(a.y, b.y, fma(c.x, d.x, c.y * d.y))), fma(a.x, b.y, fma(-a.y, b.x, fma(c.x, d.y, -c.y * d.x))));
 }
 
 struct Item {

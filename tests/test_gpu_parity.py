@@ -117,6 +117,14 @@ def test_saturated_profile_chi1024_xxz_gate():
     _synthetic_case(2, 1024, 10, 1024, profile=inputs.SATURATED_PROFILE[3], U=inputs.xxz_gate(w.delta, w.dt))
 
 
+@pytest.mark.parametrize("gate", ["identity", "swap"])
+def test_structured_gates_on_a_saturated_bond(gate):
+    """Identity and SWAP on a saturated bond: Theta(c) blocks with exact zeros and block structure (degenerate
+    rotations, rank-deficient panels, columns that are exactly orthogonal from the start)."""
+    U = np.eye(9, dtype=np.complex128) if gate == "identity" else inputs.swap_gate(3)
+    _synthetic_case(3, 240, 6, 160, U=U)
+
+
 def _synthetic_case(d, chi, R, keep_chi, profile=None, U=None):
     M, N, s, lam, gam = inputs.synthetic_gate_state(d, chi, R, seed=1234 + chi, profile=profile)
     rng = np.random.default_rng(99 + chi)
