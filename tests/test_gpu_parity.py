@@ -283,3 +283,27 @@ def test_svd_trace_and_convergence_bookkeeping():
     assert np.all(tr["sweep_ms"] > 0)
     assert tr["rotated_items"][0] > 0 and tr["inner_sweeps"][0] >= tr["rotated_items"][0]
     assert tr["active_sectors"][-1] == 0 and np.all(np.diff(tr["active_sectors"]) <= 0)
+
+
+def test_largest_local_dimension_and_vacuum():
+    """d = U1MPS_D_MAX = 8 (rows(c) spans 8 left sectors) against the oracle, and the N = 0 chain (one 1 x 1 sector
+    everywhere: the degenerate case of every kernel)."""
+    d, M, N, chi = 8, 4, 10, 96
+    occ = [3, 2, 4, 1]
+    ora = Oracle.product_state(M, d, N, chi, occ)
+    gpu = make_gpu(M, d, N, chi)
+    gpu.set_product_state(occ)
+    rng = np.random.default_rng(8)
+    for t in range(4):
+        for s in inputs.column_sites(M, t):
+            U = inputs.random_u1_gate(rng, d)
+            ora.apply_gate(s, U, chi=chi, cutoff=1e-12)
+            gpu.apply_and_truncate(s, U, chi=chi, cutoff=1e-12)
+    assert_observables(ora, gpu)
+    assert gpu.last_stats()["converged"]
+    vac = make_gpu(4, 2, 0, 4)
+    vac.set_product_state([0, 0, 0, 0])
+    vac.apply_gate_column([0, 2], np.stack([inputs.hardcore_haar_gate(rng)] * 2))
+    vac.apply_and_truncate(1, inputs.hardcore_haar_gate(rng))
+    assert np.allclose(vac.expect_n_all(), 0.0, atol=1e-15)
+    assert list(vac.bond_dims()) == [1] * 5 and abs(vac.norm2() - 1.0) < 1e-14
