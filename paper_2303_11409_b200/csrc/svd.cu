@@ -75,6 +75,7 @@ struct Item {
   int m, mt;      // rows of G; m + n = leading dimension
   int ca, na;     // first column / number of columns of panel a
   int cb, nb;     // ... of panel b (nb = 0: single-panel item)
+  const int* col; // [32] shared memory: physical column of each of the item's columns (logical order = sorted by initial norm)
   double tol2;
 };
 
@@ -87,8 +88,7 @@ __device__ __forceinline__ void load_chunk(cplx* st, int ld, const Item& I, int 
   for (int it = 0; it < SV_W * SV_R / SV_GROUP; ++it) {
     const int j = gtid / SV_R + it * (SV_GROUP / SV_R);
     const bool ok = rok && (j < U1_PB ? j < I.na : j - U1_PB < I.nb);
-    const long long gcol = j < U1_PB ? I.ca + j : I.cb + j - U1_PB;
-    const cplx* src = ok ? I.W + gcol * I.mt + row0 + r : I.W;
+    const cplx* src = ok ? I.W + (long long)I.col[j] * I.mt + row0 + r : I.W;
     cp_async16(st + j * ld + r, src, ok ? 16 : 0);
   }
 }
@@ -359,7 +359,7 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
   for (int t = 0; t < 2; ++t) {
     const int j = 8 * tj + 2 * lk + t;
     cok[t] = j < U1_PB ? j < I.na : j - U1_PB < I.nb;
-    gcol[t] = (j < U1_PB ? I.ca + j : I.cb + j - U1_PB) * (long long)I.mt;
+    gcol[t] = (long long)I.col[j] * I.mt;
   }
   const int nch = (I.mt + SV_R - 1) / SV_R;
   load_chunk(stages, SV_LDU, I, 0, I.mt, gtid);
@@ -399,6 +399,7 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
 __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S, Plan P, int G, int inner_max) {
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ unsigned s_ticket;
+  __shared__ int s_col[SV_NGROUP][SV_W];
   const int tid = threadIdx.x, g = tid / SV_GROUP, gtid = tid % SV_GROUP;
   cplx* stages = reinterpret_cast<cplx*>(smraw + (size_t)g * SV_GROUP_BYTES);
   cplx* Hs = stages;                               // [32*33], aliased onto the ring (idle during the EVD)
@@ -458,6 +459,15 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
       }
       int todo = 0, big = 0;
       if (have) {
+        // logical -> physical columns: the order of the initial column norms (descending), so that the sweeps start
+        // from a sorted matrix; the rotations keep exchanging logical columns, the map itself never changes
+        if (gtid < SV_W) {
+          const int j = gtid;
+          const bool ok = j < U1_PB ? j < I.na : j - U1_PB < I.nb;
+          s_col[g][j] = ok ? P.perm[P.svoff[e] + (j < U1_PB ? I.ca + j : I.cb + j - U1_PB)] : 0;
+        }
+        I.col = s_col[g];
+        gsync(g);
         gram_phase(stages, Hs, I, g, gtid);
         // quick test, same entries and arithmetic as the rotations: anything to do?
         for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
@@ -584,6 +594,10 @@ cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchC
   // tuning knob for experiments only: inner EVD sweeps per item, default SV_INNER_MAX
   static int inner_max = getenv("U1MPS_INNER_MAX") ? atoi(getenv("U1MPS_INNER_MAX")) : SV_INNER_MAX;
   void* args[] = {&s, &p, &gcount, &inner_max};
+  // column norms of Theta sorted descending -> P.perm: the logical column order of the Jacobi iteration
+  L.prof->begin(U1_ST_SORT, L.stream);
+  sigma_sort_kernel<<<L.sms * 2, SORT_THREADS, U1MPS_SORT_MAX * 12, L.stream>>>(P);
+  L.prof->end(L.stream);
   L.prof->begin(U1_ST_SVD, L.stream);
   cudaError_t err = cudaLaunchCooperativeKernel((void*)svd_kernel, dim3(L.svd_grid), dim3(U1_SVD_THREADS), args,
                                                 (size_t)L.svd_smem, L.stream);
@@ -592,6 +606,6 @@ cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchC
   L.prof->begin(U1_ST_SORT, L.stream);
   sigma_sort_kernel<<<L.sms * 2, SORT_THREADS, U1MPS_SORT_MAX * 12, L.stream>>>(P);
   L.prof->end(L.stream);
-  *L.launches += 2;
+  *L.launches += 3;
   return cudaGetLastError();
 }
