@@ -5,8 +5,9 @@
 // m >= n, J = identity) are made mutually orthogonal; then sigma_j = |G_j|, left vectors
 // G_j / sigma_j, right vectors J_j.
 //
-// Blocking.  Columns are grouped in panels of U1_PB = 16.  A work item is a panel pair P = [Pa Pb]
-// (32 columns):
+// Blocking.  Columns are taken in the order of their initial norms (a norm + sort pre-pass fills the logical ->
+// physical column map; the matrix is not permuted) and grouped in panels of U1_PB = 16.  A work item is a panel
+// pair P = [Pa Pb] (32 columns):
 //   1. Gram   H = P^H P over the m rows of G           (FP64 DMMA.8x8x4 tiles, chunks of 32 rows staged
 //                                                        in shared memory by a 2-stage cp.async ring)
 //   2. EVD    H = Q diag Q^H by two-sided Jacobi in shared memory (16 disjoint rotations per round on
