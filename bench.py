@@ -200,6 +200,24 @@ def dist_max(values, world, device):
     return [float(x) for x in t]
 
 
+def memory_stages(prof, work, work_after, steps):
+    """Achieved GB/s of the memory-bound a5 scatter: algorithmic bytes (read V, W out of the workspace + write the two
+    new Gammas = the Gamma bytes of the layer) / its summed CUDA-event time; against the measured
+    copy bandwidth of MEASURED_PEAKS.json.  At chi <= 1024 the per-gate working set is L2-resident."""
+    ms, n = prof.get("a5_scatter", (0.0, 0))
+    if ms <= 0:
+        return None
+    by = 0.5 * (work["gamma_bytes"] + work_after["gamma_bytes"]) * steps
+    hbm = None
+    try:
+        hbm = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        pass
+    gbs = by / (ms * 1e-3) / 1e9
+    return {"a5_scatter": {"achieved": gbs, "unit": "GB/s", "peak": hbm, "frac": (gbs / hbm) if hbm else None,
+                           "bytes_per_step": by / steps, "ms_per_step": ms / steps}}
+
+
 def svd_traffic_bytes():
     """DRAM bytes (read + write) of ONE a3 launch from the committed ncu --set full capture, or None."""
     try:
@@ -384,6 +402,7 @@ def run_ours(args, w):
                      "ms_per_launch": svd_ms / max(svd_n, 1), "launches": svd_n,
                      "share_of_step": svd_ms / ms if ms > 0 else None},
         "useful_gflops": useful_flops_step * args.steps * world / (ms * 1e-3) / 1e9,
+        "memory_bound_stages": memory_stages(prof, work, work_after, args.steps),
         "useful_frac_of_fp64_peak": useful_flops_step * args.steps * world / (ms * 1e-3) / 1e12 / (peak * world),
         "stage_ms_per_step": stage_ms,
         "trajectory": {"gates": prep_gates, "ms": prep_ms, "gates_per_s": prep_gates / (prep_ms * 1e-3) if prep_ms > 0 else None},

@@ -123,16 +123,61 @@ __global__ void __launch_bounds__(SEL_THREADS) select_kernel(DevState S, Plan P,
   }
 }
 
+// a5 tile list over (entry, part) restricted to the KEPT singular vectors (the planner sized it for all min(rows, cols)
+// of them before a4 had decided): V(c) rows x keep, W(c) keep x cols.  One CTA, exclusive scan into P.t5pref.
+__global__ void __launch_bounds__(SEL_THREADS) retile_kernel(Plan P, int L /* = 2 G NC */) {
+  __shared__ int sh[SEL_THREADS];
+  auto tiles = [&](int f) {
+    const int e = f >> 1, k = P.keep[e];
+    if (k == 0) return 0;
+    return (f & 1) ? u1_ceil_div(k, U1_TILE) * u1_ceil_div(P.cols[e], U1_TILE) : u1_ceil_div(P.rows[e], U1_TILE) * u1_ceil_div(k, U1_TILE);
+  };
+  const int t = threadIdx.x;
+  const int per = (L + SEL_THREADS - 1) / SEL_THREADS;
+  const int lo = min(L, t * per), hi = min(L, lo + per);
+  int sum = 0;
+  for (int i = lo; i < hi; ++i) sum += tiles(i);
+  sh[t] = sum;
+  __syncthreads();
+  for (int off = 1; off < SEL_THREADS; off <<= 1) {  // Hillis-Steele inclusive scan
+    const int v = (t >= off) ? sh[t - off] : 0;
+    __syncthreads();
+    sh[t] += v;
+    __syncthreads();
+  }
+  int run = sh[t] - sum;
+  for (int i = lo; i < hi; ++i) { P.t5pref[i] = run; run += tiles(i); }
+  if (t == SEL_THREADS - 1) { P.t5pref[L] = sh[t]; P.cnt[5] = sh[t]; }
+}
+
 #define SC_THREADS 256
+#define SC_RUN 16
+// a5: 32 x 32 tiles of V(c) (part 0) and W(c) (part 1) out of the stacked Jacobi matrices into the block-sparse Gammas.
+// Per tile, 64 threads first work out what is constant along a tile row / column (source column and 1/sigma of the 32
+// singular vectors; destination block, offset and 1/lambda of the 32 bond indices) into shared memory, so that the
+// two bulk passes are load - multiply - store only: coalesced 512-byte column segments in, 512-byte row segments out.
 __global__ void __launch_bounds__(SC_THREADS) scatter_kernel(DevState S, Plan P, int G) {
   __shared__ cplx tile[U1_TILE][U1_TILE + 1];
+  __shared__ long long s_src[U1_TILE];   // per singular vector jj: offset of its column in the stacked matrix (-1: not kept)
+  __shared__ double s_isg[U1_TILE];      // ... 1/sigma (or 1 where the vectors are the unit-norm J columns)
+  __shared__ long long s_dst[U1_TILE];   // per bond index (row a of V / column b of W): destination offset (-1: outside)
+  __shared__ double s_ilm[U1_TILE];      // ... 1/lambda of that bond index (Eq.13/14)
+  __shared__ int s_ldd[U1_TILE];         // ... row length of the destination block (part 1)
   const int NC = S.NC, d = S.d;
   const int nf = G * NC * 2, total = P.cnt[5];
   const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
-  for (int t = blockIdx.x; t < total; t += gridDim.x) {
+  // tiles are handed out in runs of SC_RUN consecutive tiles: one binary search of the tile prefix per run (13 dependent
+  // L2 loads), then a linear advance
+  for (int run = blockIdx.x; run * SC_RUN < total; run += gridDim.x) {
+   int f = 0;
+   {
     int lo = 0, hi = nf;
-    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (P.t5pref[mid] <= t) lo = mid; else hi = mid; }
-    const int f = lo, e = f >> 1, part = f & 1;
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (P.t5pref[mid] <= run * SC_RUN) lo = mid; else hi = mid; }
+    f = lo;
+   }
+   for (int t = run * SC_RUN; t < min(total, (run + 1) * SC_RUN); ++t) {
+    while (P.t5pref[f + 1] <= t) ++f;
+    const int e = f >> 1, part = f & 1;
     const int g = e / NC, c = e % NC, s = P.site[g];
     const int rows = P.rows[e], cols = P.cols[e], m = max(rows, cols), n = min(rows, cols), ld = m + n;
     const bool tr = rows < cols;
@@ -140,63 +185,84 @@ __global__ void __launch_bounds__(SC_THREADS) scatter_kernel(DevState S, Plan P,
     const int local = t - P.t5pref[f];
     const cplx* W = P.W + P.goff[e];
     const int so = P.svoff[e];
+    const int tcols = u1_ceil_div(part == 0 ? keep : cols, U1_TILE);
+    // part 0: tile rows = bond indices a of the left bond, tile columns = singular vectors; part 1: the other way round
+    const int x0 = (local / tcols) * U1_TILE, y0 = (local % tcols) * U1_TILE;
+    const int j0 = part == 0 ? y0 : x0, i0 = part == 0 ? x0 : y0;
+    if (j0 >= keep) continue;  // (block-uniform)
+    __syncthreads();
+    if (tid < U1_TILE) {  // singular vector j0 + tid
+      const int pj = j0 + tid;
+      long long src = -1; double isg = 1.0;
+      if (pj < keep) {
+        src = (long long)P.perm[so + pj] * ld;
+        // V = G / sigma when G holds Theta (rows >= cols), W = conj(G) / sigma when it holds Theta^H
+        if ((part == 0) != tr) isg = 1.0 / P.svs[so + pj];
+      }
+      s_src[tid] = src; s_isg[tid] = isg;
+    } else if (tid < 2 * U1_TILE) {  // bond index i0 + (tid - 32): row a of V (left bond) or column b of W (right bond)
+      const int k = tid - U1_TILE, idx = i0 + k;
+      long long dst = -1; double ilm = 0.0; int ldd = 0;
+      if (part == 0 && idx < rows) {
+        const int* nbL = S.nb + (long long)s * NC;
+        int i = 0, al = idx;
+        while (al >= nbL[c + i]) { al -= nbL[c + i]; ++i; }
+        const int cl = c + i;
+        ilm = 1.0 / S.lam[(long long)s * S.chi + S.ob[(long long)s * NC + cl] + al];
+        dst = (long long)s * S.gcap + S.gamoff[((long long)s * NC + cl) * d + i] + (long long)al * keep;
+        ldd = keep;
+      } else if (part == 1 && idx < cols) {
+        const int* nbR = S.nb + (long long)(s + 2) * NC;
+        int jq = d - 1, bl = idx;
+        while (c - jq < 0) --jq;
+        while (bl >= nbR[c - jq]) { bl -= nbR[c - jq]; --jq; }
+        const int cr = c - jq;
+        ilm = 1.0 / S.lam[(long long)(s + 2) * S.chi + S.ob[(long long)(s + 2) * NC + cr] + bl];
+        dst = (long long)(s + 1) * S.gcap + S.gamoff[((long long)(s + 1) * NC + c) * d + (c - cr)] + bl;
+        ldd = nbR[cr];
+      }
+      s_dst[k] = dst; s_ilm[k] = ilm; s_ldd[k] = ldd;
+    }
+    __syncthreads();
     if (part == 0) {
-      // V(c)[a, jj]: case A (rows >= cols) = G[a, p] / sigma_p ; case B = J[a, p]
-      const int tcols = u1_ceil_div(n, U1_TILE);
-      const int a0 = (local / tcols) * U1_TILE, j0 = (local % tcols) * U1_TILE;
-      if (j0 >= keep) continue;
-      __syncthreads();
+      // V(c)[a, jj] = G[a, p] / sigma (rows >= cols) or J[a, p]: read 32 rows of 32 columns, transpose, write rows
+      const int roff = tr ? m : 0;
       for (int jj = ty; jj < U1_TILE; jj += SC_THREADS / 32) {
-        const int pj = j0 + jj, a = a0 + tx;
         cplx v = make_double2(0.0, 0.0);
-        if (pj < keep && a < rows) {
-          const int p = P.perm[so + pj];
-          if (!tr) { const double is = 1.0 / P.svs[so + pj]; v = __ldcg(W + (long long)p * ld + a); v.x *= is; v.y *= is; }
-          else v = __ldcg(W + (long long)p * ld + m + a);
+        const long long src = s_src[jj];
+        if (src >= 0 && i0 + tx < rows) {
+          v = __ldcg(W + src + roff + i0 + tx);
+          const double sc = s_isg[jj];
+          v.x *= sc; v.y *= sc;
         }
         tile[jj][tx] = v;
       }
       __syncthreads();
-      const int* nbL = S.nb + (long long)s * NC;
       for (int aa = ty; aa < U1_TILE; aa += SC_THREADS / 32) {
-        const int a = a0 + aa, pj = j0 + tx;
-        if (a < rows && pj < keep) {
-          int i = 0, al = a;
-          while (al >= nbL[c + i]) { al -= nbL[c + i]; ++i; }
-          const int cl = c + i;
-          const double il = 1.0 / S.lam[(long long)s * S.chi + S.ob[(long long)s * NC + cl] + al];
+        const long long dst = s_dst[aa];
+        if (dst >= 0 && j0 + tx < keep) {
           cplx v = tile[tx][aa];
+          const double il = s_ilm[aa];
           v.x *= il; v.y *= il;
-          S.gam[(long long)s * S.gcap + S.gamoff[((long long)s * NC + cl) * d + i] + (long long)al * keep + pj] = v;
+          S.gam[dst + j0 + tx] = v;
         }
       }
     } else {
-      // W(c)[jj, b]: case A = conj(J[b, p]) ; case B = conj(G[b, p]) / sigma_p
-      const int tcols = u1_ceil_div(cols, U1_TILE);
-      const int j0 = (local / tcols) * U1_TILE, b0 = (local % tcols) * U1_TILE;
-      if (j0 >= keep) continue;
-      const int* nbR = S.nb + (long long)(s + 2) * NC;
-      const int b = b0 + tx;
-      int cr = 0, bl = b;
-      if (b < cols) {
-        int jq = d - 1;
-        while (c - jq < 0) --jq;
-        while (bl >= nbR[c - jq]) { bl -= nbR[c - jq]; --jq; }
-        cr = c - jq;
-      }
+      // W(c)[jj, b] = conj(J[b, p]) (rows >= cols) or conj(G[b, p]) / sigma: no transposition needed
+      const int roff = tr ? 0 : m;
+      const long long dst = s_dst[tx];
+      const double il = s_ilm[tx];
+      const int ldd = s_ldd[tx];
       for (int jj = ty; jj < U1_TILE; jj += SC_THREADS / 32) {
-        const int pj = j0 + jj;
-        if (pj < keep && b < cols) {
-          const int p = P.perm[so + pj];
-          cplx v;
-          if (!tr) v = __ldcg(W + (long long)p * ld + m + b);
-          else { const double is = 1.0 / P.svs[so + pj]; v = __ldcg(W + (long long)p * ld + b); v.x *= is; v.y *= is; }
-          const double il = 1.0 / S.lam[(long long)(s + 2) * S.chi + S.ob[(long long)(s + 2) * NC + cr] + bl];
-          v.x *= il; v.y *= -il;
-          S.gam[(long long)(s + 1) * S.gcap + S.gamoff[((long long)(s + 1) * NC + c) * d + (c - cr)] + (long long)pj * nbR[cr] + bl] = v;
+        const long long src = s_src[jj];
+        if (src >= 0 && dst >= 0) {
+          cplx v = __ldcg(W + src + roff + i0 + tx);
+          const double sc = s_isg[jj] * il;
+          S.gam[dst + (long long)(j0 + jj) * ldd] = make_double2(v.x * sc, -v.y * sc);
         }
       }
     }
+   }
   }
 }
 
@@ -206,7 +272,8 @@ void u1_launch_select_scatter(const DevState& S, const Plan& P, int G, int chi, 
   select_kernel<<<G, SEL_THREADS, S.NC * sizeof(int), L.stream>>>(S, P, G, chi, cutoff, counter, P.gate_w);
   L.prof->end(L.stream);
   L.prof->begin(U1_ST_SCATTER, L.stream);
-  scatter_kernel<<<L.sms * 4, SC_THREADS, 0, L.stream>>>(S, P, G);
+  retile_kernel<<<1, SEL_THREADS, 0, L.stream>>>(P, 2 * G * S.NC);
+  scatter_kernel<<<L.sms * 8, SC_THREADS, 0, L.stream>>>(S, P, G);
   L.prof->end(L.stream);
-  *L.launches += 2;
+  *L.launches += 3;
 }
