@@ -403,6 +403,9 @@ def run_ours(args, w):
                      "share_of_step": svd_ms / ms if ms > 0 else None},
         "useful_gflops": useful_flops_step * args.steps * world / (ms * 1e-3) / 1e9,
         "memory_bound_stages": memory_stages(prof, work, work_after, args.steps),
+        "a2_contract": {"useful_tflops": (0.5 * (work["a2_flops"] + work_after["a2_flops"]) * args.steps
+                                          / (prof["a2_contract"][0] * 1e-3) / 1e12) if prof["a2_contract"][0] > 0 else None,
+                        "note": "minimum-form flops 8 nL nC nR per (c_l, c', c_r) triple / summed CUDA-event time of contract_kernel"},
         "useful_frac_of_fp64_peak": useful_flops_step * args.steps * world / (ms * 1e-3) / 1e12 / (peak * world),
         "stage_ms_per_step": stage_ms,
         "trajectory": {"gates": prep_gates, "ms": prep_ms, "gates_per_s": prep_gates / (prep_ms * 1e-3) if prep_ms > 0 else None},

@@ -12,6 +12,7 @@
 
 #define KC 16          // K-chunk (columns of A / rows of B) per stage
 #define CT_THREADS 128 // 4 warps: warp w owns rows 8w..8w+7 of the 32 x 32 output tile (4 DMMA tiles of 8 x 8)
+#define CT_RUN 4       // consecutive tiles per work-queue step
 #define CT_LD 34       // shared-memory leading dimension (complex elements), 2 mod 8: conflict-free LDS.128 fragments
 
 __device__ __forceinline__ cplx cmul(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -39,8 +40,12 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P
   const int nf = G * NC * dd;
   const int total = P.cnt[4];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, lr = lane >> 2, lk = lane & 3;
-  for (int tile = blockIdx.x; tile < total; tile += gridDim.x) {
-    const int f = upper_entry(P.t2pref, nf, tile);
+  // tiles are handed out in runs of CT_RUN consecutive tiles: one binary search of the tile prefix per run, then a
+  // linear advance
+  for (int run = blockIdx.x; run * CT_RUN < total; run += gridDim.x) {
+   int f = upper_entry(P.t2pref, nf, run * CT_RUN);
+   for (int tile = run * CT_RUN; tile < min(total, (run + 1) * CT_RUN); ++tile) {
+    while (P.t2pref[f + 1] <= tile) ++f;
     const int e = f / dd, i = (f / d) % d, j = f % d;
     const int g = e / NC, c = e % NC, s = P.site[g];
     const int cl = c + i, cr = c - j;
@@ -141,6 +146,7 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P
           }
         }
     }
+   }
   }
 }
 
