@@ -220,7 +220,9 @@ def parabolic_profile(chi: int, R: int) -> List[int]:
 
 # sector sizes of a saturated bond of config 3 (XXZ, chi = 1024) as measured on the trajectory after 50 layers
 # (DESIGN.md section 4); used so that the CPU-baseline sample has the block sizes of the real workload
-SATURATED_PROFILE = {3: (5, 32, 100, 195, 256, 229, 139, 54, 13, 1)}
+SATURATED_PROFILE = {3: (5, 32, 100, 195, 256, 229, 139, 54, 13, 1),
+                     # config 5 (beam splitters, d = 4, chi = 4096), bond 50 after 16 columns
+                     5: (2, 18, 77, 229, 460, 686, 809, 758, 550, 311, 138, 47, 10, 1)}
 
 
 def synthetic_gate_state(d: int, chi: int, R: int, seed: int, decay: float = 0.97, profile=None):

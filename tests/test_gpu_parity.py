@@ -117,6 +117,14 @@ def test_saturated_profile_chi1024_xxz_gate():
     _synthetic_case(2, 1024, 10, 1024, profile=inputs.SATURATED_PROFILE[3], U=inputs.xxz_gate(w.delta, w.dt))
 
 
+def test_saturated_profile_chi4096_beam_splitter_gate():
+    """Largest size of BASELINE.json (config 5): d = 4, chi = 4096, the sector sizes measured on its trajectory
+    (Theta(c) blocks up to ~2800 x 2800, 175 panels), one Haar beam-splitter gate, every sigma, V sigma W and the kept
+    set against the oracle (about 25 s, most of it LAPACK in the oracle)."""
+    U = inputs.haar_beam_splitter_gate(np.random.default_rng(55), 4)
+    _synthetic_case(4, 4096, 14, 4096, profile=inputs.SATURATED_PROFILE[5], U=U)
+
+
 @pytest.mark.parametrize("gate", ["identity", "swap"])
 def test_structured_gates_on_a_saturated_bond(gate):
     """Identity and SWAP on a saturated bond: Theta(c) blocks with exact zeros and block structure (degenerate
