@@ -33,6 +33,9 @@ namespace cg = cooperative_groups;
 #define SV_HLD 33                    // leading dimension of the 32 x 32 Gram matrix (row-major)
 static_assert(U1_MAXSWEEP == 30, "keep U1MPS_MAXSWEEP of include/u1mps.h in step");
 #define SV_QLD 36                    // leading dimension of the transposed eigenvector matrix Qt (4 mod 8: B fragments)
+#ifndef SV_TOLFAC
+#define SV_TOLFAC 8.0                // stopping threshold tol = SV_TOLFAC eps sqrt(m) on |h_pq| / sqrt(h_pp h_qq)
+#endif
 #define SV_INNER_MAX 2               // inner EVD sweeps per item (the outer iteration finishes the job; measured best of 1..4)
 #define SV_LASTPASS 1e-18            // (relative off-diagonal)^2 below which a rotation needs no verification sweep
 #define SV_QUAD 1e-14                // stop the inner EVD after a sweep whose largest relative off-diagonal^2 was below this
@@ -455,7 +458,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
         I.W = P.W + P.goff[e];
         I.ca = pa * U1_PB; I.na = min(U1_PB, n - I.ca);
         I.cb = pb * U1_PB; I.nb = pb < np ? min(U1_PB, n - I.cb) : 0;
-        const double tol = 8.0 * 1.1102230246251565e-16 * sqrt((double)I.m);
+        const double tol = SV_TOLFAC * 1.1102230246251565e-16 * sqrt((double)I.m);
         I.tol2 = tol * tol;
       }
       int todo = 0, big = 0;
