@@ -315,3 +315,60 @@ def test_largest_local_dimension_and_vacuum():
     vac.apply_and_truncate(1, inputs.hardcore_haar_gate(rng))
     assert np.allclose(vac.expect_n_all(), 0.0, atol=1e-15)
     assert list(vac.bond_dims()) == [1] * 5 and abs(vac.norm2() - 1.0) < 1e-14
+
+
+def test_column_of_saturated_gates_chi1024():
+    """The launch configuration bench.py times: SEVERAL saturated chi = 1024 gates in ONE column call (one launch of
+    every kernel for all of them: shared plan, work lists and Jacobi rounds), each with the sector sizes measured on
+    config 3 and its own random blocks; every gate's kept table, lambda~ and gauge-invariant product
+    lamL Gamma~ lam~ Gamma~ lamR against the oracle applied gate by gate."""
+    d, chi, ng = 2, 1024, 4
+    w3 = inputs.WORKLOADS[3]
+    U = inputs.xxz_gate(w3.delta, w3.dt)
+    states = [inputs.synthetic_gate_state(d, chi, 10, seed=500 + g, profile=inputs.SATURATED_PROFILE[3]) for g in range(ng)]
+    N = states[0][1]
+    M = 4 * ng + 2
+    occ, left = [0] * M, N
+    for i in range(M):
+        occ[i] = min(d - 1, left)
+        left -= occ[i]
+    assert left == 0
+    ora = Oracle.product_state(M, d, N, chi, occ)
+    sites = []
+    for g, (_, _, _, lam, gam) in enumerate(states):
+        s = 2 + 4 * g
+        sites.append(s)
+        for k in (0, 1, 2):
+            ora.sectors[s + k] = sorted(lam[2 + k])
+            ora.lam[s + k] = lam[2 + k]
+        ora.gam[s] = gam[2]
+        ora.gam[s + 1] = gam[3]
+    ws_gate = 2 * d * chi * chi * 16
+    from paper_2303_11409_b200.binding import load_library
+    need = load_library().u1mps_workspace_bytes(M, d, N, chi)
+    gpu = make_gpu(M, d, N, chi, arena_bytes=need + ng * ws_gate)
+    gpu.set_product_state(occ)
+    for s in sites:
+        oracle_to_gpu(ora, gpu, bonds=[s, s + 1, s + 2], sites=[s, s + 1])
+    launches0 = gpu.launch_count()
+    gpu.apply_gate_column(sites, np.stack([U] * ng), chi=chi, cutoff=1e-12)
+    assert gpu.launch_count() - launches0 == 9          # one launch of every kernel for the whole column
+    assert gpu.last_stats()["converged"]
+    for g, s in enumerate(sites):
+        lamL, lamR = states[g][3][2], states[g][3][4]
+        rec = ora.apply_gate(s, U, chi=chi, cutoff=1e-12, record=True)
+        want_tab = {c: k for c, k in rec.keep.items() if k > 0}
+        assert dict(gpu.bond_info(s + 1)) == want_tab
+        lam_new = gpu.export_bond(s + 1)
+        sig1 = max(float(rec.sigma[c][0]) for c in rec.charges)
+        for c in want_tab:
+            assert np.max(np.abs(lam_new[c] - ora.lam[s + 1][c])) <= 1e-10 * max(1.0, sig1)
+        g_s, g_s1 = gpu.export_site(s), gpu.export_site(s + 1)
+        wk, fro = rec.weight_kept, np.sqrt(rec.weight_all)
+        for c, kc in want_tab.items():
+            want = (rec.V[c][:, :kc] * rec.sigma[c][None, :kc]) @ rec.W[c][:kc, :] / np.sqrt(wk)
+            got = np.zeros_like(want)
+            for cl, ro, nr in rec.rows[c]:
+                for cr, co, ncol in rec.cols[c]:
+                    got[ro:ro + nr, co:co + ncol] = (lamL[cl][:, None] * g_s[(cl, c)] * lam_new[c][None, :]) @ (g_s1[(c, cr)] * lamR[cr][None, :])
+            assert np.linalg.norm(got - want) <= 1e-10 * fro / np.sqrt(wk), (g, c)
