@@ -38,7 +38,7 @@ static_assert(U1_MAXSWEEP == 30, "keep U1MPS_MAXSWEEP of include/u1mps.h in step
 #endif
 #define SV_INNER_MAX 2               // inner EVD sweeps per item (the outer iteration finishes the job; measured best of 1..4)
 #define SV_LASTPASS 1e-18            // (relative off-diagonal)^2 below which a rotation needs no verification sweep
-#define SV_QUAD 1e-14                // stop the inner EVD after a sweep whose largest relative off-diagonal^2 was below this
+#define SV_QUAD 1e-4                 // no second inner sweep after one whose largest relative off-diagonal^2 was below this (measured best of 1e-14 .. 3e-1)
 #define SV_GROUP 128                 // threads per pair item (= one CTA: SV_NGROUP == 1; several groups per CTA were tried and dropped)
 #define SV_NGROUP (U1_SVD_THREADS / SV_GROUP)
 #define SV_CTAS 6                    // resident CTAs per SM the kernel is compiled for (registers <= 85)
