@@ -221,8 +221,10 @@ def memory_stages(prof, work, work_after, steps):
 def svd_traffic_bytes():
     """DRAM bytes (read + write) of ONE a3 launch from the committed ncu --set full capture, or None."""
     try:
-        d = json.load(open(os.path.join(ROOT, "profiles", "svd_traffic.json")))
-        return float(d["dram_bytes_read"]) + float(d["dram_bytes_write"])
+        import csv
+        with open(os.path.join(ROOT, "profiles", "svd_traffic.csv")) as f:
+            row = next(csv.DictReader(f))
+        return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
     except Exception:
         return None
 
@@ -397,7 +399,7 @@ def run_ours(args, w):
                      "frac": achieved / peak, "traffic": svd_traffic_bytes(),
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA/clk x 2 x sm_max_mhz (no FP64 entry in MEASURED_PEAKS.json; "
                                     "the round-1 probe measured 36.8 DFMA / 37.06 DMMA TFLOP/s, DESIGN.md section 6)",
-                     "traffic_source": "profiles/svd_traffic.json (ncu --set full, one launch of the same workload)",
+                     "traffic_source": "profiles/svd_traffic.csv (ncu --set full, one launch of the same workload)",
                      "flops": "useful SVD flops 4*min(14mn^2+8n^3, 6mn^2+20n^3) per block (SURVEY §8(d))",
                      "ms_per_launch": svd_ms / max(svd_n, 1), "launches": svd_n,
                      "share_of_step": svd_ms / ms if ms > 0 else None},
