@@ -105,7 +105,8 @@ int u1mps_bond_entropy_all(u1mps_t* h, double* out_host /*[M+1]*/);
 int u1mps_bond_info(u1mps_t* h, int bond, int32_t* n_sectors, int32_t* charges, int32_t* counts, int cap);
 int u1mps_bond_dims(u1mps_t* h, int32_t* dims_host /*[M+1]*/);
 /* Statistics since create / set_product_state: total discarded weight; of the LAST column or
- * gate: kept bond dimension of its first gate, Jacobi sweeps used (max over sectors). */
+ * gate: kept bond dimension of its first gate, Jacobi sweeps used by its slowest sector (a sweep = one visit of every
+ * panel pair of the largest sector; U1MPS_ENOCONV is returned if some sector needed more than U1MPS_MAXSWEEP). */
 int u1mps_last_stats(u1mps_t* h, double* discarded_weight, int* kept, int* sweeps);
 
 /* Export / import (teacher-forced parity, checkpoints).  All [sync]; host buffers. */
@@ -137,8 +138,9 @@ int u1mps_profile_read(u1mps_t* h, double* ms_host, long long* launches_host);
 const char* u1mps_stage_name(int stage); /* "a1_plan", "a2_contract", ... ; "" if out of range */
 
 /* Trace of the LAST a3 launch (one column or gate) [sync]: out_host[0] = start time, then 4 arrays of U1MPS_MAXSWEEP
- * entries: end time of each Jacobi sweep (GPU globaltimer, ns), pair items that rotated, inner EVD sweeps run, sectors
- * still active.  cap (entries of out_host) must be >= 4 * U1MPS_MAXSWEEP + 1. */
+ * entries, one per Jacobi sweep (= np_max rounds of the modulus ordering, np_max = panels of the largest sector of the
+ * launch): end time (GPU globaltimer, ns), panel-pair items that rotated, inner EVD sweeps run, sectors not yet
+ * converged at the end of the sweep.  cap (entries of out_host) must be >= 4 * U1MPS_MAXSWEEP + 1. */
 #define U1MPS_MAXSWEEP 30
 int u1mps_svd_trace(u1mps_t* h, long long* out_host, int cap);
 
