@@ -128,7 +128,7 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
     const cplx* pb0 = st + 8 * tb[0] * SV_LDG;
     const cplx* pb1 = st + 8 * tb[1] * SV_LDG;
     const cplx* pb2 = st + 8 * tb[2] * SV_LDG;
-#pragma unroll 2
+#pragma unroll 1
     for (int ks = 0; ks < nk; ++ks) {
       const cplx a0 = pa0[4 * ks], a1 = pa1[4 * ks], b0 = pb0[4 * ks], b1 = pb1[4 * ks];
       // conj(a) * b : re = ar br + ai bi ; im = ar bi - ai br
