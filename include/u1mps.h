@@ -16,8 +16,9 @@
  *
  * Conventions.  All functions return int: 0 = OK, negative = error (never throw, never abort).
  * "host" / "device" says where a pointer must live.  The caller owns every pointer it passes;
- * the library copies what it needs before returning (host U) or in stream order (device U: the
- * buffer must stay valid until the stream has passed the call).  The arena and the stream given
+ * host arguments (sites, host U) are copied into a library-owned pinned staging ring before the call
+ * returns and may be reused at once; a device U is read in stream order (the buffer must stay
+ * valid until the stream has passed the call).  The arena and the stream given
  * to u1mps_create are borrowed for the lifetime of the handle.  Calls marked [sync] synchronise
  * the stream; all others only enqueue work (sector sizes stay on the device).
  */
@@ -39,8 +40,13 @@ enum {
   U1MPS_ENOTU1 = -2,  /* host gate has an entry > 1e-14 that violates charge conservation (Eq.1) */
   U1MPS_ESTAGED = -3, /* call not allowed in the current staging state (see u1mps_apply_two_site_gate) */
   U1MPS_ENOMEM = -4,  /* arena too small for this call */
-  U1MPS_ECUDA = -5,   /* CUDA error (sticky), or no CUDA device */
-  U1MPS_ENOCONV = -6  /* Jacobi SVD hit the sweep limit on some sector (reported by [sync] calls) */
+  U1MPS_ECUDA = -5,   /* CUDA error, or no CUDA device.  Sticky: once a CUDA runtime call of a handle has failed, every
+                         later call on that handle returns U1MPS_ECUDA */
+  U1MPS_ENOCONV = -6  /* Jacobi SVD hit the sweep limit on some sector.  Detected on the device, so it is reported by the
+                         [sync] calls that read the device status (log_norm, norm2, last_stats, staged_info,
+                         export_staged_svd).  Sticky, like U1MPS_ENOMEM raised by a launch whose plan did not fit the arena:
+                         it stays set until u1mps_clear_status or u1mps_set_product_state, so that a failure in any gate
+                         since the last check is never lost */
 };
 
 const char* u1mps_strerror(int code);
@@ -108,6 +114,8 @@ int u1mps_bond_dims(u1mps_t* h, int32_t* dims_host /*[M+1]*/);
  * gate: kept bond dimension of its first gate, Jacobi sweeps used by its slowest sector (a sweep = one visit of every
  * panel pair of the largest sector; U1MPS_ENOCONV is returned if some sector needed more than U1MPS_MAXSWEEP). */
 int u1mps_last_stats(u1mps_t* h, double* discarded_weight, int* kept, int* sweeps);
+/* Clear the sticky device status (U1MPS_ENOCONV / device-side U1MPS_ENOMEM).  Enqueued in stream order. */
+int u1mps_clear_status(u1mps_t* h);
 
 /* Export / import (teacher-forced parity, checkpoints).  All [sync]; host buffers. */
 int u1mps_export_bond(u1mps_t* h, int bond, double* lambda_host, int cap);  /* ascending c, descending inside */

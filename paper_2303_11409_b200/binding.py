@@ -22,7 +22,7 @@ EXPORTS = [
     "u1mps_bond_dims", "u1mps_last_stats", "u1mps_export_bond", "u1mps_export_site", "u1mps_import_bond",
     "u1mps_import_site", "u1mps_set_log_norm", "u1mps_staged_info", "u1mps_export_staged_theta",
     "u1mps_export_staged_svd", "u1mps_launch_count", "u1mps_profile_enable", "u1mps_profile_read",
-    "u1mps_stage_name", "u1mps_svd_trace",
+    "u1mps_stage_name", "u1mps_svd_trace", "u1mps_clear_status",
 ]
 NSTAGE = 8
 
@@ -83,6 +83,7 @@ def load_library() -> C.CDLL:
     lib.u1mps_profile_enable.argtypes = [vp, C.c_int]
     lib.u1mps_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
     lib.u1mps_svd_trace.argtypes = [vp, C.POINTER(C.c_longlong), C.c_int]
+    lib.u1mps_clear_status.argtypes = [vp]
     lib.u1mps_stage_name.restype = C.c_char_p
     lib.u1mps_stage_name.argtypes = [C.c_int]
     for name in EXPORTS:
@@ -183,15 +184,19 @@ class U1MPS:
                                                   self.chi if chi is None else chi, cutoff))
 
     # ------------------------------------------------------------------ readouts
-    def norm2(self) -> float:
+    def norm2(self, allow_nonconverged: bool = False) -> float:
+        """Raises U1MPSError(ENOCONV) if any SVD since the last clear_status() hit the sweep limit (unless allowed)."""
         v = C.c_double()
-        self._ck(self.lib.u1mps_norm2(self.h, C.byref(v)), allow=(ENOCONV,))
+        self._ck(self.lib.u1mps_norm2(self.h, C.byref(v)), allow=(ENOCONV,) if allow_nonconverged else ())
         return v.value
 
-    def log_norm(self) -> float:
+    def log_norm(self, allow_nonconverged: bool = False) -> float:
         v = C.c_double()
-        self._ck(self.lib.u1mps_log_norm(self.h, C.byref(v)), allow=(ENOCONV,))
+        self._ck(self.lib.u1mps_log_norm(self.h, C.byref(v)), allow=(ENOCONV,) if allow_nonconverged else ())
         return v.value
+
+    def clear_status(self):
+        self._ck(self.lib.u1mps_clear_status(self.h))
 
     def expect_n(self, site: int) -> float:
         v = C.c_double()

@@ -83,6 +83,12 @@ struct u1mps {
   cudaError_t cuda_err;
   std::vector<int> h_nb;           // host copy of the tables (filled by sync calls)
   std::vector<long long> h_gamoff; // host copy of one site's block offsets
+  // library-owned pinned staging ring for host arguments (sites, host gates): the caller's buffers are copied here before
+  // the call returns, the H2D copies are asynchronous and a slot is reused only after its copy has completed
+  static const int NSLOT = 4;
+  char* stg = nullptr; size_t stg_slot = 0; int stg_next = 0;
+  cudaEvent_t stg_ev[NSLOT] = {nullptr, nullptr, nullptr, nullptr};
+  bool stg_busy[NSLOT] = {false, false, false, false};
 };
 
 namespace {
@@ -96,6 +102,27 @@ int cuda_fail(u1mps* h, cudaError_t e) {
     cudaError_t _e = (call);                            \
     if (_e != cudaSuccess) return cuda_fail(h, _e);     \
   } while (0)
+
+// a slot of the pinned staging ring with room for `bytes` (grows the ring if needed; waits for the slot's last copy)
+int staging_slot(u1mps* h, size_t bytes, char** out, int* slot) {
+  if (bytes > h->stg_slot) {
+    CK(cudaStreamSynchronize(h->stream));
+    if (h->stg) { cudaFreeHost(h->stg); h->stg = nullptr; h->stg_slot = 0; }
+    const size_t sz = (bytes + 4095) & ~(size_t)4095;
+    CK(cudaHostAlloc((void**)&h->stg, sz * u1mps::NSLOT, cudaHostAllocDefault));
+    h->stg_slot = sz;
+    for (int i = 0; i < u1mps::NSLOT; ++i) {
+      h->stg_busy[i] = false;
+      if (!h->stg_ev[i]) CK(cudaEventCreateWithFlags(&h->stg_ev[i], cudaEventDisableTiming));
+    }
+  }
+  const int k = h->stg_next;
+  h->stg_next = (k + 1) % u1mps::NSLOT;
+  if (h->stg_busy[k]) { CK(cudaEventSynchronize(h->stg_ev[k])); h->stg_busy[k] = false; }
+  *out = h->stg + (size_t)k * h->stg_slot;
+  *slot = k;
+  return U1MPS_OK;
+}
 
 int check_device_flags(u1mps* h) {  // after a sync
   int err[3];
@@ -135,8 +162,20 @@ int check_u1_host(const double* U, int d) {
 // upload sites + gates of one chunk and run a1-a2 (and a3 if with_svd)
 int run_front(u1mps* h, const int32_t* sites, int G, const void* U, int on_dev, bool with_svd) {
   const size_t ubytes = (size_t)G * h->d * h->d * h->d * h->d * sizeof(cplx);
-  CK(cudaMemcpyAsync(h->P.site, sites, (size_t)G * 4, cudaMemcpyHostToDevice, h->stream));
-  CK(cudaMemcpyAsync(h->P.U, U, ubytes, on_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+  const size_t sbytes = ((size_t)G * 4 + 255) & ~(size_t)255;
+  char* stg; int slot;
+  int r = staging_slot(h, sbytes + (on_dev ? 0 : ubytes), &stg, &slot);
+  if (r) return r;
+  std::memcpy(stg, sites, (size_t)G * 4);
+  CK(cudaMemcpyAsync(h->P.site, stg, (size_t)G * 4, cudaMemcpyHostToDevice, h->stream));
+  if (on_dev) {
+    CK(cudaMemcpyAsync(h->P.U, U, ubytes, cudaMemcpyDeviceToDevice, h->stream));
+  } else {
+    std::memcpy(stg + sbytes, U, ubytes);
+    CK(cudaMemcpyAsync(h->P.U, stg + sbytes, ubytes, cudaMemcpyHostToDevice, h->stream));
+  }
+  CK(cudaEventRecord(h->stg_ev[slot], h->stream));
+  h->stg_busy[slot] = true;
   u1_launch_plan(h->S, h->P, G, h->L);
   u1_launch_contract(h->S, h->P, G, h->L);
   if (with_svd) CK(u1_launch_svd(h->S, h->P, G, h->L));
@@ -229,6 +268,10 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
   if (e == cudaSuccess) e = cudaMemsetAsync(P.cnt, 0, 8 * 4, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(S.err, 0, 8 * 4, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(S.scal, 0, 8 * 8, h->stream);
+  // empty bond tables and block offsets: a fresh handle may be filled by the import calls alone
+  if (e == cudaSuccess) e = cudaMemsetAsync(S.nb, 0, (size_t)(M + 1) * NC * 4, h->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(S.ob, 0, (size_t)(M + 1) * NC * 4, h->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(S.gamoff, 0, (size_t)M * NC * d * 8, h->stream);
   if (e != cudaSuccess) { delete h; return U1MPS_ECUDA; }
   h->L.sms = sms; h->L.svd_grid = grid; h->L.svd_smem = smem; h->L.stream = h->stream; h->L.launches = &h->launches; h->L.prof = &h->prof;
   *out = h;
@@ -239,11 +282,14 @@ int u1mps_destroy(u1mps_t* h) {
   if (!h) return U1MPS_EINVAL;
   cudaStreamSynchronize(h->stream);
   h->prof.destroy();
+  for (int i = 0; i < u1mps::NSLOT; ++i) if (h->stg_ev[i]) cudaEventDestroy(h->stg_ev[i]);
+  if (h->stg) cudaFreeHost(h->stg);
   delete h;
   return U1MPS_OK;
 }
 
 int u1mps_set_product_state(u1mps_t* h, const int32_t* occ) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !occ) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
   long long tot = 0;
@@ -257,6 +303,7 @@ int u1mps_set_product_state(u1mps_t* h, const int32_t* occ) {
 }
 
 static int stage_common(u1mps_t* h, int i, const void* U, int on_dev, bool with_svd) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !U || i < 0 || i > h->M - 2) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
   if (!on_dev) { int r = check_u1_host((const double*)U, h->d); if (r) return r; }
@@ -274,6 +321,7 @@ int u1mps_apply_two_site_gate(u1mps_t* h, int i, const void* U, int on_dev) { re
 int u1mps_stage_theta(u1mps_t* h, int i, const void* U, int on_dev) { return stage_common(h, i, U, on_dev, false); }
 
 int u1mps_stage_svd(u1mps_t* h) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h) return U1MPS_EINVAL;
   if (h->stage != ST_THETA) return U1MPS_ESTAGED;
   CK(u1_launch_svd(h->S, h->P, 1, h->L));
@@ -282,6 +330,7 @@ int u1mps_stage_svd(u1mps_t* h) {
 }
 
 int u1mps_truncate(u1mps_t* h, int i, int chi, double cutoff) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || chi < 1 || chi > h->chi || !(cutoff >= 0.0)) return U1MPS_EINVAL;
   if (h->stage != ST_SVD || h->staged_site != i) return U1MPS_ESTAGED;
   int32_t site = i;
@@ -298,6 +347,7 @@ int u1mps_apply_and_truncate(u1mps_t* h, int i, const void* U, int on_dev, int c
 }
 
 int u1mps_apply_gate_column(u1mps_t* h, const int32_t* sites, int n, const void* U, int on_dev, int chi, double cutoff) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !sites || !U || n < 1 || chi < 1 || chi > h->chi || !(cutoff >= 0.0)) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
   for (int g = 0; g < n; ++g) {
@@ -330,13 +380,22 @@ int u1mps_apply_gate_column(u1mps_t* h, const int32_t* sites, int n, const void*
   return U1MPS_OK;
 }
 
+int u1mps_clear_status(u1mps_t* h) {
+  if (!h) return U1MPS_EINVAL;
+  if (h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // CUDA errors are not recoverable
+  CK(cudaMemsetAsync(h->S.err, 0, 3 * 4, h->stream));
+  return U1MPS_OK;
+}
+
 int u1mps_log_norm(u1mps_t* h, double* out) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out) return U1MPS_EINVAL;
   CK(cudaMemcpyAsync(out, h->S.scal, 8, cudaMemcpyDeviceToHost, h->stream));
   return check_device_flags(h);
 }
 
 int u1mps_norm2(u1mps_t* h, double* out) {
+  if (!out) return U1MPS_EINVAL;
   double ln = 0.0;
   int r = u1mps_log_norm(h, &ln);
   if (r && r != U1MPS_ENOCONV) return r;
@@ -345,6 +404,7 @@ int u1mps_norm2(u1mps_t* h, double* out) {
 }
 
 int u1mps_expect_n_all(u1mps_t* h, double* out) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
   u1_launch_expect_n(h->S, h->dout, h->L);
@@ -355,6 +415,7 @@ int u1mps_expect_n_all(u1mps_t* h, double* out) {
 }
 
 int u1mps_expect_n(u1mps_t* h, int site, double* out) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out || site < 0 || site >= h->M) return U1MPS_EINVAL;
   std::vector<double> all(h->M);
   int r = u1mps_expect_n_all(h, all.data());
@@ -364,6 +425,7 @@ int u1mps_expect_n(u1mps_t* h, int site, double* out) {
 }
 
 int u1mps_bond_entropy_all(u1mps_t* h, double* out) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
   u1_launch_entropy(h->S, h->dout, h->L);
@@ -374,6 +436,7 @@ int u1mps_bond_entropy_all(u1mps_t* h, double* out) {
 }
 
 int u1mps_bond_entropy(u1mps_t* h, int bond, double* out) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out || bond < 0 || bond > h->M) return U1MPS_EINVAL;
   std::vector<double> all(h->M + 1);
   int r = u1mps_bond_entropy_all(h, all.data());
@@ -383,6 +446,7 @@ int u1mps_bond_entropy(u1mps_t* h, int bond, double* out) {
 }
 
 int u1mps_bond_info(u1mps_t* h, int bond, int32_t* n_sectors, int32_t* charges, int32_t* counts, int cap) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !n_sectors || bond < 0 || bond > h->M) return U1MPS_EINVAL;
   int r = sync_tables(h);
   if (r) return r;
@@ -398,6 +462,7 @@ int u1mps_bond_info(u1mps_t* h, int bond, int32_t* n_sectors, int32_t* charges, 
 }
 
 int u1mps_bond_dims(u1mps_t* h, int32_t* dims) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !dims) return U1MPS_EINVAL;
   int r = sync_tables(h);
   if (r) return r;
@@ -410,6 +475,7 @@ int u1mps_bond_dims(u1mps_t* h, int32_t* dims) {
 }
 
 int u1mps_last_stats(u1mps_t* h, double* discarded, int* kept, int* sweeps) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h) return U1MPS_EINVAL;
   double sc[4]; int err[3];
   CK(cudaMemcpyAsync(sc, h->S.scal, sizeof(sc), cudaMemcpyDeviceToHost, h->stream));
@@ -428,6 +494,7 @@ int u1mps_last_stats(u1mps_t* h, double* discarded, int* kept, int* sweeps) {
 }
 
 int u1mps_export_bond(u1mps_t* h, int bond, double* lam, int cap) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !lam || bond < 0 || bond > h->M) return U1MPS_EINVAL;
   int r = sync_tables(h);
   if (r) return r;
@@ -452,6 +519,7 @@ static int site_block(u1mps_t* h, int site, int cl, int cr, long long* off, long
 }
 
 int u1mps_export_site(u1mps_t* h, int site, int cl, int cr, void* block, size_t cap) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !block) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
   long long off, nl, nr;
@@ -464,6 +532,7 @@ int u1mps_export_site(u1mps_t* h, int site, int cl, int cr, void* block, size_t 
 }
 
 int u1mps_import_bond(u1mps_t* h, int bond, int nsec, const int32_t* charges, const int32_t* counts, const double* lam) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !charges || !counts || !lam || bond < 0 || bond > h->M || nsec < 1) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
   std::vector<int> nb(h->NC, 0), ob(h->NC, 0);
@@ -476,19 +545,26 @@ int u1mps_import_bond(u1mps_t* h, int bond, int nsec, const int32_t* charges, co
   if (D > h->chi) return U1MPS_EINVAL;
   int run = 0;
   for (int c = 0; c < h->NC; ++c) { ob[c] = run; run += nb[c]; }
+  // validate against the neighbouring bonds BEFORE anything is overwritten: the blocks of sites bond-1 and bond must fit
+  int r = sync_tables(h);
+  if (r) return r;
+  std::copy(nb.begin(), nb.end(), h->h_nb.begin() + (size_t)bond * h->NC);
+  long long used[2] = {0, 0};
+  const int s_lo = std::max(0, bond - 1), s_hi = std::min(h->M - 1, bond);
+  for (int s = s_lo; s <= s_hi; ++s) {
+    long long u = 0;
+    for (int cl = 0; cl < h->NC; ++cl)
+      for (int i = 0; i < h->d && cl - i >= 0; ++i)
+        u += (long long)h->h_nb[(size_t)s * h->NC + cl] * h->h_nb[(size_t)(s + 1) * h->NC + cl - i];
+    if (u > h->S.gcap) return U1MPS_EINVAL;
+    used[s - s_lo] = u;
+  }
   CK(cudaMemcpyAsync(h->S.nb + (size_t)bond * h->NC, nb.data(), (size_t)h->NC * 4, cudaMemcpyHostToDevice, h->stream));
   CK(cudaMemcpyAsync(h->S.ob + (size_t)bond * h->NC, ob.data(), (size_t)h->NC * 4, cudaMemcpyHostToDevice, h->stream));
   CK(cudaMemcpyAsync(h->S.lam + (size_t)bond * h->chi, lam, (size_t)D * 8, cudaMemcpyHostToDevice, h->stream));
   h->Dh[bond] = D;
-  int r = sync_tables(h);
-  if (r) return r;
-  for (int s = std::max(0, bond - 1); s <= std::min(h->M - 1, bond); ++s) {
-    long long used = 0;
-    for (int cl = 0; cl < h->NC; ++cl)
-      for (int i = 0; i < h->d && cl - i >= 0; ++i)
-        used += (long long)h->h_nb[(size_t)s * h->NC + cl] * h->h_nb[(size_t)(s + 1) * h->NC + cl - i];
-    if (used > h->S.gcap) return U1MPS_EINVAL;
-    CK(cudaMemsetAsync(h->S.gam + (size_t)s * h->S.gcap, 0, (size_t)used * sizeof(cplx), h->stream));
+  for (int s = s_lo; s <= s_hi; ++s) {
+    CK(cudaMemsetAsync(h->S.gam + (size_t)s * h->S.gcap, 0, (size_t)used[s - s_lo] * sizeof(cplx), h->stream));
     u1_launch_gamoff(h->S, s, h->L);
   }
   CK(cudaGetLastError());
@@ -497,6 +573,7 @@ int u1mps_import_bond(u1mps_t* h, int bond, int nsec, const int32_t* charges, co
 }
 
 int u1mps_import_site(u1mps_t* h, int site, int cl, int cr, const void* block, size_t bytes) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !block) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
   long long off, nl, nr;
@@ -509,6 +586,7 @@ int u1mps_import_site(u1mps_t* h, int site, int cl, int cr, const void* block, s
 }
 
 int u1mps_set_log_norm(u1mps_t* h, double log_norm, double discarded) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h) return U1MPS_EINVAL;
   double v[2] = {log_norm, discarded};
   CK(cudaMemcpyAsync(h->S.scal, v, 16, cudaMemcpyHostToDevice, h->stream));
@@ -526,6 +604,7 @@ static int staged_rc(u1mps_t* h, std::vector<int>& rows, std::vector<int>& cols)
 }
 
 int u1mps_staged_info(u1mps_t* h, int32_t* n_cand, int32_t* charges, int32_t* rows, int32_t* cols, int cap) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !n_cand) return U1MPS_EINVAL;
   if (h->stage == ST_NONE) return U1MPS_ESTAGED;
   std::vector<int> r, q;
@@ -559,6 +638,7 @@ static int fetch_block(u1mps_t* h, int c, std::vector<cplx>& buf, int* rows, int
 }
 
 int u1mps_export_staged_theta(u1mps_t* h, int c, void* theta, size_t cap) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !theta) return U1MPS_EINVAL;
   if (h->stage != ST_THETA) return U1MPS_ESTAGED;
   std::vector<cplx> buf; int rows, cols;
@@ -578,6 +658,7 @@ int u1mps_export_staged_theta(u1mps_t* h, int c, void* theta, size_t cap) {
 }
 
 int u1mps_export_staged_svd(u1mps_t* h, int c, void* V, double* sigma, void* Wout) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h) return U1MPS_EINVAL;
   if (h->stage != ST_SVD) return U1MPS_ESTAGED;
   std::vector<cplx> buf; int rows, cols;
@@ -621,6 +702,7 @@ int u1mps_export_staged_svd(u1mps_t* h, int c, void* V, double* sigma, void* Wou
 }
 
 int u1mps_profile_enable(u1mps_t* h, int on) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h) return U1MPS_EINVAL;
   CK(cudaStreamSynchronize(h->stream));
   h->prof.used = 0;
@@ -629,6 +711,7 @@ int u1mps_profile_enable(u1mps_t* h, int on) {
 }
 
 int u1mps_profile_read(u1mps_t* h, double* ms, long long* launches) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !ms || !launches) return U1MPS_EINVAL;
   CK(cudaStreamSynchronize(h->stream));
   for (int s = 0; s < U1MPS_NSTAGE; ++s) { ms[s] = 0.0; launches[s] = 0; }
@@ -649,6 +732,7 @@ const char* u1mps_stage_name(int stage) {
 }
 
 int u1mps_svd_trace(u1mps_t* h, long long* out, int cap) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out || cap < 4 * U1_MAXSWEEP + 1) return U1MPS_EINVAL;
   CK(cudaMemcpyAsync(out, h->P.trace, (4 * U1_MAXSWEEP + 1) * 8, cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
@@ -656,6 +740,7 @@ int u1mps_svd_trace(u1mps_t* h, long long* out, int cap) {
 }
 
 int u1mps_launch_count(u1mps_t* h, long long* out) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out) return U1MPS_EINVAL;
   *out = h->launches;
   return U1MPS_OK;

@@ -57,6 +57,36 @@ struct Plan {
 
 __host__ __device__ inline int u1_ceil_div(int a, int b) { return (a + b - 1) / b; }
 
+#ifdef __CUDACC__
+// D(8x8) += A(8x4, row) * B(4x8, col), FP64 tensor tile (SASS: DMMA.8x8x4).
+// Fragments: a = A[lane>>2][lane&3], b = B[lane&3][lane>>2], c0/c1 = C[lane>>2][2*(lane&3) + 0/1].
+__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// Exclusive scan of f(0..L-1) into out[0..L] (out[L] = total) by one CTA of NT threads; sh: NT entries of shared memory.
+template <typename T, int NT, typename F>
+__device__ void u1_block_excl_scan(F f, T* out, int L, T* sh) {
+  const int t = threadIdx.x;
+  const int per = (L + NT - 1) / NT;
+  const int lo = min(L, t * per), hi = min(L, lo + per);
+  T sum = 0;
+  for (int i = lo; i < hi; ++i) sum += f(i);
+  sh[t] = sum;
+  __syncthreads();
+  for (int off = 1; off < NT; off <<= 1) {  // Hillis-Steele inclusive scan
+    T v = (t >= off) ? sh[t - off] : (T)0;
+    __syncthreads();
+    sh[t] += v;
+    __syncthreads();
+  }
+  T run = sh[t] - sum;
+  for (int i = lo; i < hi; ++i) { T v = f(i); out[i] = run; run += v; }
+  if (t == NT - 1) out[L] = sh[t];
+  __syncthreads();
+}
+#endif
+
 // Optional per-kernel timing (u1mps_profile_*): CUDA events recorded on the handle's stream around
 // every launch of a stage; summed when read.  Host side only.
 enum { U1_ST_PLAN = 0, U1_ST_CONTRACT, U1_ST_IDENTITY, U1_ST_SVD, U1_ST_SORT, U1_ST_SELECT, U1_ST_SCATTER, U1_ST_READOUT, U1_NSTAGE };

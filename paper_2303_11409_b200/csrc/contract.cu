@@ -17,12 +17,6 @@
 
 __device__ __forceinline__ cplx cmul(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 
-// D(8x8) += A(8x4, row) * B(4x8, col), FP64 tensor tile (SASS: DMMA.8x8x4).
-// Fragments: a = A[lane>>2][lane&3], b = B[lane&3][lane>>2], c0/c1 = C[lane>>2][2*(lane&3) + 0/1].
-__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
-  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
 // largest idx in [0, n) with pref[idx] <= v  (pref non-decreasing, pref[0] = 0 <= v < pref[n])
 __device__ __forceinline__ int upper_entry(const int* __restrict__ pref, int n, int v) {
   int lo = 0, hi = n;  // invariant: pref[lo] <= v < pref[hi]

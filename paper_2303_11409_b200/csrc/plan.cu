@@ -7,35 +7,13 @@
 #define PLAN_THREADS 1024
 #define U1_MAXPANELS (U1MPS_SORT_MAX / U1_PB)   // panels of the largest sector (n <= chi <= 4096)
 
-// Exclusive scan of f(0..L-1) into out[0..L] (out[L] = total) by one CTA.
-template <typename T, typename F>
-__device__ void block_excl_scan(F f, T* out, int L, T* sh /*[PLAN_THREADS]*/) {
-  const int t = threadIdx.x;
-  const int per = (L + PLAN_THREADS - 1) / PLAN_THREADS;
-  const int lo = min(L, t * per), hi = min(L, lo + per);
-  T sum = 0;
-  for (int i = lo; i < hi; ++i) sum += f(i);
-  sh[t] = sum;
-  __syncthreads();
-  for (int off = 1; off < PLAN_THREADS; off <<= 1) {  // Hillis-Steele inclusive scan
-    T v = (t >= off) ? sh[t - off] : (T)0;
-    __syncthreads();
-    sh[t] += v;
-    __syncthreads();
-  }
-  T run = sh[t] - sum;
-  for (int i = lo; i < hi; ++i) { T v = f(i); out[i] = run; run += v; }
-  if (t == PLAN_THREADS - 1) out[L] = sh[t];
-  __syncthreads();
-}
-
 __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, int G) {
   __shared__ long long shl[PLAN_THREADS];
   __shared__ int shi[PLAN_THREADS];
-  __shared__ int shmax;
+  __shared__ int shmax, sh_over;
   __shared__ int cls_count[U1_MAXPANELS + 1], cls_fill[U1_MAXPANELS + 1], cls_base[U1_MAXPANELS + 1];
   const int NC = S.NC, d = S.d, E = G * NC, t = threadIdx.x;
-  if (t == 0) shmax = 0;
+  if (t == 0) { shmax = 0; sh_over = 0; }
   // (i)-(iii) rows(c), cols(c) of every candidate centre charge
   for (int e = t; e < E; e += PLAN_THREADS) {
     const int g = e / NC, c = e % NC, s = P.site[g];
@@ -53,15 +31,15 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
   }
   __syncthreads();
   // Theta / Jacobi workspace offsets: stacked (m+n) x n column-major, m = max(rows, cols), n = min
-  block_excl_scan<long long>(
+  u1_block_excl_scan<long long, PLAN_THREADS>(
       [&](int e) { long long r = P.rows[e], q = P.cols[e]; long long m = max(r, q), n = min(r, q); return (m + n) * n; },
       P.goff, E, shl);
-  if (t == 0 && P.goff[E] > P.wcap) atomicExch(S.err, U1_ERR_WORKSPACE);
-  block_excl_scan<int>([&](int e) { return min(P.rows[e], P.cols[e]); }, P.svoff, E, shi);
-  if (t == 0 && P.svoff[E] > P.poolcap) atomicExch(S.err, U1_ERR_WORKSPACE);
+  if (t == 0 && P.goff[E] > P.wcap) sh_over = 1;
+  u1_block_excl_scan<int, PLAN_THREADS>([&](int e) { return min(P.rows[e], P.cols[e]); }, P.svoff, E, shi);
+  if (t == 0 && P.svoff[E] > P.poolcap) sh_over = 1;
   // (iv) a2 tile list over (e, i, j): block (c_l = c+i, c_r = c-j) of Theta(c)
   const int dd = d * d;
-  block_excl_scan<int>(
+  u1_block_excl_scan<int, PLAN_THREADS>(
       [&](int f) {
         const int e = f / dd, i = (f / d) % d, j = f % d;
         if (P.rows[e] == 0) return 0;
@@ -72,7 +50,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
       },
       P.t2pref, E * dd, shi);
   // a5 tile list over (e, part): V rows x n, W n x cols
-  block_excl_scan<int>(
+  u1_block_excl_scan<int, PLAN_THREADS>(
       [&](int f) {
         const int e = f >> 1;
         const int r = P.rows[e], q = P.cols[e], n = min(r, q);
@@ -85,7 +63,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
     const int n = min(P.rows[e], P.cols[e]);
     return u1_ceil_div(n, U1_PB);
   };
-  block_excl_scan<int>([&](int e) { return min(P.rows[e], P.cols[e]) > 0 ? 1 : 0; }, P.tmpa, E, shi);
+  u1_block_excl_scan<int, PLAN_THREADS>([&](int e) { return min(P.rows[e], P.cols[e]) > 0 ? 1 : 0; }, P.tmpa, E, shi);
   for (int e = t; e < E; e += PLAN_THREADS)
     if (min(P.rows[e], P.cols[e]) > 0) P.blk[P.tmpa[e]] = e;
   if (t == 0) P.cnt[0] = P.tmpa[E];
@@ -108,7 +86,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
     P.cnt[4] = P.t2pref[E * dd];
     P.cnt[5] = P.t5pref[E * 2];
     P.cnt[6] = 0;
-    if (run > P.itemcap) atomicExch(S.err, U1_ERR_WORKSPACE);
+    if (run > P.itemcap) sh_over = 1;
   }
   __syncthreads();
   const bool ok = cls_base[0] <= P.itemcap;
@@ -125,7 +103,12 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
   for (int i = t; i < 2 * E; i += PLAN_THREADS) P.flags[i] = i < E ? 0 : 0x7fffffff;   // a3: last_rot[E], done_at[E]
   for (int i = t; i < 4 * U1_MAXSWEEP + 1; i += PLAN_THREADS) P.trace[i] = 0;
   __syncthreads();
-  if (t == 0) P.cnt[3] = shmax;
+  if (t == 0) {
+    P.cnt[3] = shmax;
+    // the plan does not fit the arena: report it, and hand every later kernel of the launch an EMPTY work list, so that
+    // nothing is written through the oversize offsets
+    if (sh_over) { atomicExch(S.err, U1_ERR_WORKSPACE); P.cnt[0] = 0; P.cnt[1] = 0; P.cnt[4] = 0; P.cnt[5] = 0; }
+  }
 }
 
 void u1_launch_plan(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {

@@ -30,6 +30,7 @@ __global__ void __launch_bounds__(SEL_THREADS) select_kernel(DevState S, Plan P,
   __shared__ double s_w[2];
   __shared__ int s_top;
   __shared__ int s_last;
+  if (S.err[0] != 0) return;   // the plan did not fit (U1_ERR_WORKSPACE): its offsets must not be used
   const int NC = S.NC, d = S.d, g = blockIdx.x, s = P.site[g], C = s + 1;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int* svo = P.svoff + g * NC;
@@ -132,22 +133,8 @@ __global__ void __launch_bounds__(SEL_THREADS) retile_kernel(Plan P, int L /* = 
     if (k == 0) return 0;
     return (f & 1) ? u1_ceil_div(k, U1_TILE) * u1_ceil_div(P.cols[e], U1_TILE) : u1_ceil_div(P.rows[e], U1_TILE) * u1_ceil_div(k, U1_TILE);
   };
-  const int t = threadIdx.x;
-  const int per = (L + SEL_THREADS - 1) / SEL_THREADS;
-  const int lo = min(L, t * per), hi = min(L, lo + per);
-  int sum = 0;
-  for (int i = lo; i < hi; ++i) sum += tiles(i);
-  sh[t] = sum;
-  __syncthreads();
-  for (int off = 1; off < SEL_THREADS; off <<= 1) {  // Hillis-Steele inclusive scan
-    const int v = (t >= off) ? sh[t - off] : 0;
-    __syncthreads();
-    sh[t] += v;
-    __syncthreads();
-  }
-  int run = sh[t] - sum;
-  for (int i = lo; i < hi; ++i) { P.t5pref[i] = run; run += tiles(i); }
-  if (t == SEL_THREADS - 1) { P.t5pref[L] = sh[t]; P.cnt[5] = sh[t]; }
+  u1_block_excl_scan<int, SEL_THREADS>(tiles, P.t5pref, L, sh);
+  if (threadIdx.x == 0) P.cnt[5] = P.t5pref[L];
 }
 
 #define SC_THREADS 256

@@ -20,7 +20,6 @@
 // on the Theta blocks of the workloads).  Convergence is decided on the device per sector (np consecutive rounds,
 // i.e. every panel pair once, without an off-diagonal Gram entry above the threshold), no host round trip.
 #include <cooperative_groups.h>
-#include <cstdlib>
 #include "common.cuh"
 namespace cg = cooperative_groups;
 
@@ -49,12 +48,6 @@ __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
-}
-
-// D(8x8) += A(8x4, row) * B(4x8, col), FP64 tensor tile (SASS: DMMA.8x8x4).
-// Fragments: a = A[lane>>2][lane&3], b = B[lane&3][lane>>2], c0/c1 = C[lane>>2][2*(lane&3) + 0/1].
-__device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
-  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem, int src_bytes) {
@@ -595,8 +588,7 @@ cudaError_t u1_svd_configure(int* grid, int* smem_bytes, int sms) {
 
 cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
   DevState s = S; Plan p = P; int gcount = G;
-  // tuning knob for experiments only: inner EVD sweeps per item, default SV_INNER_MAX
-  static int inner_max = getenv("U1MPS_INNER_MAX") ? atoi(getenv("U1MPS_INNER_MAX")) : SV_INNER_MAX;
+  int inner_max = SV_INNER_MAX;
   void* args[] = {&s, &p, &gcount, &inner_max};
   // column norms of Theta sorted descending -> P.perm: the logical column order of the Jacobi iteration
   L.prof->begin(U1_ST_SORT, L.stream);
