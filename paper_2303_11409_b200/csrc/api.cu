@@ -49,6 +49,7 @@ Sizes compute_sizes(int M, int d, int N, int chi) {
   add((E + 1) * 8); add((E + 1) * 4);                            // goff svoff
   add((E * d * d + 1) * 4); add((2 * E + 1) * 4);                // t2pref t5pref
   add(8 * 4); add(2 * E * 4); add((size_t)2 * z.Gmax * 8);  // cnt flags gate_w
+  add(U1_SCHED * 4);                                             // sched
   add((4 * U1_MAXSWEEP + 1) * 8);                                // trace
   for (int i = 0; i < 2; ++i) add((size_t)z.itemcap * 4);        // item lists
   add((size_t)z.poolcap * 4); add((size_t)z.poolcap * 8); add((size_t)z.poolcap * 8);  // perm sv svs
@@ -250,6 +251,7 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
   P.goff = A.take<long long>(E + 1); P.svoff = A.take<int>(E + 1);
   P.t2pref = A.take<int>(E * d * d + 1); P.t5pref = A.take<int>(2 * E + 1);
   P.cnt = A.take<int>(8); P.flags = A.take<int>(2 * E); P.gate_w = A.take<double>((size_t)2 * z.Gmax);
+  P.sched = A.take<int>(U1_SCHED);
   P.trace = A.take<long long>(4 * U1_MAXSWEEP + 1);
   P.pitem_e = A.take<int>(z.itemcap); P.pitem_k = A.take<int>(z.itemcap);
   P.perm = A.take<int>(z.poolcap); P.sv = A.take<double>(z.poolcap); P.svs = A.take<double>(z.poolcap);

@@ -85,7 +85,6 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
     P.cnt[1] = run;
     P.cnt[4] = P.t2pref[E * dd];
     P.cnt[5] = P.t5pref[E * 2];
-    P.cnt[6] = 0;
     if (run > P.itemcap) sh_over = 1;
   }
   __syncthreads();
@@ -102,6 +101,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
   atomicMax(&shmax, mymax);
   for (int i = t; i < 2 * E; i += PLAN_THREADS) P.flags[i] = i < E ? 0 : 0x7fffffff;   // a3: last_rot[E], done_at[E]
   for (int i = t; i < 4 * U1_MAXSWEEP + 1; i += PLAN_THREADS) P.trace[i] = 0;
+  for (int i = t; i < U1_SCHED; i += PLAN_THREADS) P.sched[i] = 0;
   __syncthreads();
   if (t == 0) {
     P.cnt[3] = shmax;

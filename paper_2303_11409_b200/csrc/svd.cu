@@ -20,6 +20,9 @@
 // on the Theta blocks of the workloads).  Convergence is decided on the device per sector (np consecutive rounds,
 // i.e. every panel pair once, without an off-diagonal Gram entry above the threshold), no host round trip.
 #include <cooperative_groups.h>
+#ifdef SV_PROFILE
+#include <cstdlib>
+#endif
 #include "common.cuh"
 namespace cg = cooperative_groups;
 
@@ -28,7 +31,13 @@ namespace cg = cooperative_groups;
 #define SV_LDG 36                    // shared-memory leading dimension (complex elements) in the Gram phase: 4 mod 8
 #define SV_LDU 34                    // ... in the update phase: 2 mod 8 (both: conflict-free LDS.128 fragment loads)
 #define SV_STAGE (SV_W * SV_LDG)     // complex elements per stage
-#define SV_NSTAGE 2
+#ifndef SV_MIN_ACTIVE
+#define SV_MIN_ACTIVE 2
+#endif
+#ifndef SV_ITEMS_PER_CTA
+#define SV_ITEMS_PER_CTA 4           // a3 throttle: items per active CTA and round below which fewer CTAs per SM are used
+#endif
+#define SV_NSTAGE 3                  // cp.async ring depth: chunks c + 1 and c + 2 are in flight while chunk c is consumed
 #define SV_HLD 33                    // leading dimension of the 32 x 32 Gram matrix (row-major)
 static_assert(U1_MAXSWEEP == 30, "keep U1MPS_MAXSWEEP of include/u1mps.h in step");
 #define SV_QLD 36                    // leading dimension of the transposed eigenvector matrix Qt (4 mod 8: B fragments)
@@ -40,7 +49,8 @@ static_assert(U1_MAXSWEEP == 30, "keep U1MPS_MAXSWEEP of include/u1mps.h in step
 #define SV_QUAD 1e-4                 // no second inner sweep after one whose largest relative off-diagonal^2 was below this (measured best of 1e-14 .. 3e-1)
 #define SV_GROUP 128                 // threads per pair item (= one CTA: SV_NGROUP == 1; several groups per CTA were tried and dropped)
 #define SV_NGROUP (U1_SVD_THREADS / SV_GROUP)
-#define SV_CTAS 6                    // resident CTAs per SM the kernel is compiled for (registers <= 85)
+#define SV_CTAS 4                    // resident CTAs per SM the kernel is compiled for (registers <= 128: no spills with the
+                                     // 3M accumulators; measured best of 3..6, profiles/r2_svd_tuning.md)
 #define SV_GROUP_BYTES (SV_NSTAGE * SV_STAGE * 16)   // 36,864 B per group
 #define SV_SMEM_BYTES (SV_NGROUP * SV_GROUP_BYTES)
 
@@ -102,16 +112,23 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
   ta[0] = warp == 0 ? 0 : warp == 1 ? 3 : warp == 2 ? 1 : 2;  tb[0] = warp == 0 ? 0 : warp == 1 ? 0 : warp == 2 ? 1 : 2;
   ta[1] = warp == 0 ? 0 : warp == 1 ? 3 : warp == 2 ? 1 : 3;  tb[1] = warp == 0 ? 1 : warp == 1 ? 1 : warp == 2 ? 2 : 3;
   ta[2] = warp == 0 ? 0 : 3;                                   tb[2] = 2;
-  double cre[3][2], cim[3][2];
+  // complex products with three real tile products instead of four (3M): for conj(a) b
+  //   T1 = ar br, T2 = ai bi, T3 = (ar - ai)(br + bi);  re = T1 + T2, im = T3 - T1 + T2
+  // (normwise as accurate as the four-product form: every term is bounded by |a||b|)
+  double t1[3][2], t2[3][2], t3[3][2];
 #pragma unroll
-  for (int u = 0; u < 3; ++u) { cre[u][0] = cre[u][1] = 0.0; cim[u][0] = cim[u][1] = 0.0; }
+  for (int u = 0; u < 3; ++u) { t1[u][0] = t1[u][1] = 0.0; t2[u][0] = t2[u][1] = 0.0; t3[u][0] = t3[u][1] = 0.0; }
   const int nch = (I.m + SV_R - 1) / SV_R;
-  load_chunk(stages, SV_LDG, I, 0, I.m, gtid);
-  cp_async_commit();
+#pragma unroll
+  for (int p = 0; p < SV_NSTAGE - 1; ++p) {
+    if (p < nch) load_chunk(stages + p * SV_STAGE, SV_LDG, I, p * SV_R, I.m, gtid);
+    cp_async_commit();
+  }
   for (int c = 0; c < nch; ++c) {
-    cp_async_wait<0>();
+    cp_async_wait<SV_NSTAGE - 2>();
     gsync(g);  // chunk c has landed for everybody, and everybody is done with chunk c - 1: its stage may be refilled
-    if (c + 1 < nch) load_chunk(stages + ((c + 1) % SV_NSTAGE) * SV_STAGE, SV_LDG, I, (c + 1) * SV_R, I.m, gtid);
+    if (c + SV_NSTAGE - 1 < nch)
+      load_chunk(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDG, I, (c + SV_NSTAGE - 1) * SV_R, I.m, gtid);
     cp_async_commit();
     const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE + lr * SV_LDG + lk;
     const int rows = min(SV_R, I.m - c * SV_R);
@@ -124,18 +141,20 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
 #pragma unroll 1
     for (int ks = 0; ks < nk; ++ks) {
       const cplx a0 = pa0[4 * ks], a1 = pa1[4 * ks], b0 = pb0[4 * ks], b1 = pb1[4 * ks];
-      // conj(a) * b : re = ar br + ai bi ; im = ar bi - ai br
-      dmma(cre[0][0], cre[0][1], a0.x, b0.x); dmma(cre[0][0], cre[0][1], a0.y, b0.y);
-      dmma(cim[0][0], cim[0][1], a0.x, b0.y); dmma(cim[0][0], cim[0][1], -a0.y, b0.x);
-      dmma(cre[1][0], cre[1][1], a1.x, b1.x); dmma(cre[1][0], cre[1][1], a1.y, b1.y);
-      dmma(cim[1][0], cim[1][1], a1.x, b1.y); dmma(cim[1][0], cim[1][1], -a1.y, b1.x);
+      const double a0d = a0.x - a0.y, a1d = a1.x - a1.y;
+      dmma(t1[0][0], t1[0][1], a0.x, b0.x); dmma(t2[0][0], t2[0][1], a0.y, b0.y); dmma(t3[0][0], t3[0][1], a0d, b0.x + b0.y);
+      dmma(t1[1][0], t1[1][1], a1.x, b1.x); dmma(t2[1][0], t2[1][1], a1.y, b1.y); dmma(t3[1][0], t3[1][1], a1d, b1.x + b1.y);
       if (nt == 3) {  // warp-uniform; the A tile of slot 2 is that of slot 0
         const cplx b2 = pb2[4 * ks];
-        dmma(cre[2][0], cre[2][1], a0.x, b2.x); dmma(cre[2][0], cre[2][1], a0.y, b2.y);
-        dmma(cim[2][0], cim[2][1], a0.x, b2.y); dmma(cim[2][0], cim[2][1], -a0.y, b2.x);
+        dmma(t1[2][0], t1[2][1], a0.x, b2.x); dmma(t2[2][0], t2[2][1], a0.y, b2.y); dmma(t3[2][0], t3[2][1], a0d, b2.x + b2.y);
       }
     }
   }
+  double cre[3][2], cim[3][2];
+#pragma unroll
+  for (int u = 0; u < 3; ++u)
+#pragma unroll
+    for (int t = 0; t < 2; ++t) { cre[u][t] = t1[u][t] + t2[u][t]; cim[u][t] = (t3[u][t] - t1[u][t]) + t2[u][t]; }
   cp_async_wait<0>();
   gsync(g);  // every warp is done with the stages: Hs (aliased onto the ring) may be written
 #pragma unroll
@@ -159,6 +178,9 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
   gsync(g);
 }
 
+__device__ __forceinline__ double rsqrt_approx(double x) { double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
+__device__ __forceinline__ double rcp_approx(double x) { double y; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
+
 // pivot k of round t of the round-robin tournament over np2 players (not ordered: consecutive k give consecutive
 // indices, which keeps the shared-memory accesses of a quarter warp in distinct banks)
 __device__ __forceinline__ void pivot(int t, int k, int np2, int* p, int* q) {
@@ -169,8 +191,6 @@ __device__ __forceinline__ void pivot(int t, int k, int np2, int* p, int* q) {
   if (b >= m) b -= m;
   *p = a; *q = b;
 }
-__device__ __forceinline__ double rsqrt_approx(double x) { double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
-__device__ __forceinline__ double rcp_approx(double x) { double y; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
 
 // ---- phase 2: two-sided Jacobi EVD of the Hermitian H (2*hp x 2*hp, hp = 16 or 8 pivots per round), Qt (stored
 // transposed) accumulates the rotations; both in place in shared memory.
@@ -343,11 +363,12 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
   const int lane = gtid & 31, warp = gtid >> 5;
   const int tj = warp;
   const int lr = lane >> 2, lk = lane & 3;
-  double bre[8], bim[8];
+  // 3M complex products: T1 = ar br, T2 = ai bi, T3 = (ar + ai)(br + bi);  re = T1 - T2, im = T3 - T1 - T2
+  double bre[8], bim[8], bsm[8];
 #pragma unroll
   for (int ks = 0; ks < 8; ++ks) {
     const cplx v = Qt[(8 * tj + lr) * SV_QLD + 4 * ks + lk];   // Q[k][j], k = 4 ks + lk, j = 8 tj + lr
-    bre[ks] = v.x; bim[ks] = v.y;
+    bre[ks] = v.x; bim[ks] = v.y; bsm[ks] = v.x + v.y;
   }
   gsync(g);  // Q (aliased onto the ring) is in registers everywhere: the ring may be refilled
   // the two output columns of this lane
@@ -359,12 +380,16 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
     gcol[t] = (long long)I.col[j] * I.mt;
   }
   const int nch = (I.mt + SV_R - 1) / SV_R;
-  load_chunk(stages, SV_LDU, I, 0, I.mt, gtid);
-  cp_async_commit();
+#pragma unroll
+  for (int p = 0; p < SV_NSTAGE - 1; ++p) {
+    if (p < nch) load_chunk(stages + p * SV_STAGE, SV_LDU, I, p * SV_R, I.mt, gtid);
+    cp_async_commit();
+  }
   for (int c = 0; c < nch; ++c) {
-    cp_async_wait<0>();
+    cp_async_wait<SV_NSTAGE - 2>();
     gsync(g);  // chunk c has landed for everybody, and everybody is done with chunk c - 1: its stage may be refilled
-    if (c + 1 < nch) load_chunk(stages + ((c + 1) % SV_NSTAGE) * SV_STAGE, SV_LDU, I, (c + 1) * SV_R, I.mt, gtid);
+    if (c + SV_NSTAGE - 1 < nch)
+      load_chunk(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDU, I, (c + SV_NSTAGE - 1) * SV_R, I.mt, gtid);
     cp_async_commit();
     const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE;
     const int row0 = c * SV_R;
@@ -372,20 +397,17 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
 #pragma unroll
     for (int rt = 0; rt < SV_R / 8; ++rt) {
       if (8 * rt >= rows) break;
-      double cre[2] = {0.0, 0.0}, cim[2] = {0.0, 0.0};
+      double u1[2] = {0.0, 0.0}, u2[2] = {0.0, 0.0}, u3[2] = {0.0, 0.0};
       const cplx* pa = st + lk * SV_LDU + 8 * rt + lr;
 #pragma unroll
       for (int ks = 0; ks < 8; ++ks) {
         const cplx a = pa[4 * ks * SV_LDU];
-        const double nai = -a.y;
-        // a * b : re = ar br - ai bi ; im = ar bi + ai br
-        dmma(cre[0], cre[1], a.x, bre[ks]); dmma(cre[0], cre[1], nai, bim[ks]);
-        dmma(cim[0], cim[1], a.x, bim[ks]); dmma(cim[0], cim[1], a.y, bre[ks]);
+        dmma(u1[0], u1[1], a.x, bre[ks]); dmma(u2[0], u2[1], a.y, bim[ks]); dmma(u3[0], u3[1], a.x + a.y, bsm[ks]);
       }
       const int r = row0 + 8 * rt + lr;
       if (r < I.mt) {
-        if (cok[0]) I.W[gcol[0] + r] = make_double2(cre[0], cim[0]);
-        if (cok[1]) I.W[gcol[1] + r] = make_double2(cre[1], cim[1]);
+        if (cok[0]) I.W[gcol[0] + r] = make_double2(u1[0] - u2[0], (u3[0] - u1[0]) - u2[0]);
+        if (cok[1]) I.W[gcol[1] + r] = make_double2(u1[1] - u2[1], (u3[1] - u1[1]) - u2[1]);
       }
     }
   }
@@ -393,7 +415,7 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
   gsync(g);
 }
 
-__global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S, Plan P, int G, int inner_max) {
+__global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S, Plan P, int G, int inner_max, int sms) {
   extern __shared__ __align__(16) unsigned char smraw[];
   __shared__ unsigned s_ticket;
   __shared__ int s_col[SV_NGROUP][SV_W];
@@ -410,14 +432,31 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
   const int E = G * S.NC;
   int* last_rot = P.flags;                         // [E] round after the last rotation outside the quadratic regime
   int* done_at = P.flags + E;                      // [E] round at which the sector was found converged (INT_MAX: not yet)
-  unsigned base = 0;
-  unsigned* ticket = reinterpret_cast<unsigned*>(P.cnt + 6);
+  // Load-dependent throttle: a round hands its items to only as many CTAs per SM as the work warrants (the CTAs of an
+  // SM share the FP64 pipe, the shared-memory pipe and the issue slots: with few items per round every resident CTA beyond
+  // what is needed only slows the others down; measured in profiles/r2_svd_tuning.md).  Each CTA learns its rank on its SM
+  // once; the number of active ranks of the next round follows from the items that did work in this one.
+  int* sched = P.sched;   // [0..2] items that did work in round t (mod 3), [3..5] work-queue tickets (mod 3), [8 + smid] ranks
+  __shared__ int s_rank;
+  if (tid == 0) { unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid)); s_rank = atomicAdd(&sched[8 + (smid & 255)], 1); }
+  __syncthreads();
+  const int rank = s_rank;
+  auto active_ranks = [&](int items) { return min(SV_CTAS, max(SV_MIN_ACTIVE, (items + SV_ITEMS_PER_CTA * sms - 1) / (SV_ITEMS_PER_CTA * sms))); };
+  int kact = active_ranks(npair);
   if (blockIdx.x == 0 && tid == 0) { long long t0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0)); P.trace[0] = t0; }
   int tg = 0, n_rot = 0, n_inner = 0, ndone = 0;
+#ifdef SV_PROFILE   // debug build only: clock64 per phase, summed over the grid into the tail of the trace
+  long long pc[6] = {0, 0, 0, 0, 0, 0}, pt = clock64();
+#define SV_TICK(k) do { const long long _n = clock64(); pc[k] += _n - pt; pt = _n; } while (0)
+#else
+#define SV_TICK(k) do {} while (0)
+#endif
   for (; tg < U1_MAXSWEEP * R && nblk > 0; ++tg) {
-    for (;;) {
+    unsigned* ticket = reinterpret_cast<unsigned*>(sched + 3 + tg % 3);
+    int worked = 0;
+    for (; rank < kact;) {
       __syncthreads();
-      if (tid == 0) s_ticket = atomicAdd(ticket, (unsigned)SV_NGROUP) - base;
+      if (tid == 0) s_ticket = atomicAdd(ticket, (unsigned)SV_NGROUP);
       __syncthreads();
       const unsigned it0 = s_ticket;
       if (it0 >= (unsigned)npair) break;
@@ -455,6 +494,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
         I.tol2 = tol * tol;
       }
       int todo = 0, big = 0;
+      worked += have ? 1 : 0;
       if (have) {
         // logical -> physical columns: the order of the initial column norms (descending), so that the sweeps start
         // from a sorted matrix; the rotations keep exchanging logical columns, the map itself never changes
@@ -465,7 +505,9 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
         }
         I.col = s_col[g];
         gsync(g);
+        SV_TICK(0);
         gram_phase(stages, Hs, I, g, gtid);
+        SV_TICK(1);
         // quick test, same entries and arithmetic as the rotations: anything to do?
         for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
           const int p = idx >> 5, qq = idx & 31;
@@ -486,16 +528,24 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
         if (big && gtid == 0) atomicMax(&last_rot[e], tg + 1);
       }
       __syncthreads();
+      SV_TICK(0);
       int inner = 0;
       if (todo) evd_phase(Hs, Qs, Rm, tab, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
       __syncthreads();
+      SV_TICK(2);
       if (todo) {
         update_phase(stages, Qs, I, g, gtid);
         if (gtid == 0) { n_rot += 1; n_inner += inner; }
       }
+      SV_TICK(3);
     }
-    base += (unsigned)SV_NGROUP * ((unsigned)(npair + SV_NGROUP - 1) / SV_NGROUP + gridDim.x);
+    SV_TICK(0);
+    if (tid == 0 && worked) atomicAdd(&sched[tg % 3], worked);
     grid.sync();
+    SV_TICK(4);
+    // the counters of round tg + 2 (last read after the grid sync of round tg - 1, which every CTA has left behind)
+    if (blockIdx.x == 0 && tid == 0) { sched[(tg + 2) % 3] = 0; sched[3 + (tg + 2) % 3] = 0; }
+    kact = active_ranks(__ldcg(&sched[tg % 3]));
     // ---- convergence: sectors found finished up to this round (stamps of later rounds are ignored, so that every
     // CTA takes the same decision)
     int mine = 0;
@@ -522,6 +572,9 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
     }
     if (last) { ++tg; break; }
   }
+#ifdef SV_PROFILE
+  if (tid == 0) for (int k = 0; k < 5; ++k) atomicAdd((unsigned long long*)&P.trace[1 + 3 * U1_MAXSWEEP + 20 + k], (unsigned long long)pc[k]);
+#endif
   if (blockIdx.x == 0 && tid == 0) {
     atomicMax(&S.err[1], (tg + R - 1) / R);
     if (nblk > 0 && ndone < nblk) atomicAdd(&S.err[2], nblk - ndone);
@@ -589,13 +642,18 @@ cudaError_t u1_svd_configure(int* grid, int* smem_bytes, int sms) {
 cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchCfg& L) {
   DevState s = S; Plan p = P; int gcount = G;
   int inner_max = SV_INNER_MAX;
-  void* args[] = {&s, &p, &gcount, &inner_max};
+  int sms = L.sms;
+  void* args[] = {&s, &p, &gcount, &inner_max, &sms};
   // column norms of Theta sorted descending -> P.perm: the logical column order of the Jacobi iteration
   L.prof->begin(U1_ST_SORT, L.stream);
   sigma_sort_kernel<<<L.sms * 2, SORT_THREADS, U1MPS_SORT_MAX * 12, L.stream>>>(P);
   L.prof->end(L.stream);
+  int grid = L.svd_grid;
+#ifdef SV_PROFILE   // debug build only: CTAs per SM from the environment (phase latencies without contention)
+  if (getenv("SV_PROFILE_CTAS")) grid = L.sms * atoi(getenv("SV_PROFILE_CTAS"));
+#endif
   L.prof->begin(U1_ST_SVD, L.stream);
-  cudaError_t err = cudaLaunchCooperativeKernel((void*)svd_kernel, dim3(L.svd_grid), dim3(U1_SVD_THREADS), args,
+  cudaError_t err = cudaLaunchCooperativeKernel((void*)svd_kernel, dim3(grid), dim3(U1_SVD_THREADS), args,
                                                 (size_t)L.svd_smem, L.stream);
   L.prof->end(L.stream);
   if (err != cudaSuccess) return err;
