@@ -206,6 +206,9 @@ __device__ __forceinline__ void pivot(int t, int k, int np2, int* p, int* q) {
 // sides and written, together with its mirror image, by one thread (H stays exactly Hermitian); the Q units
 // (two rows x the two columns of a pivot) likewise.  The pivots of a round come from a small shared-memory table of the
 // modulus ordering (pairs with (i + j) mod 2hp == round), the same pipelined cyclic-by-rows ordering as the outer one.
+#ifdef EVD_CLK
+__device__ long long evd_clk[20];
+#endif
 struct Rot { double cs, sr, si; int flag; };   // flag: 0 idle, 1 rotate, 3 rotate and exchange
 __device__ __forceinline__ Rot load_rot(const double4* Rm, int k) {
   const double4 v = Rm[k];
@@ -254,37 +257,90 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
       uki = ki; ukj = ki + 1 + u;
     }
   }
-  // this thread's Q units: rows (rp, rp + hp) x pivots kq0 and kq0 + 8 (hp = 16), or pivot kq0 only (hp = 8, tid < 64)
-  const int rp = tid % hp, kq0 = tid / hp;
-  const int nq = (hp == U1_PB) ? 2 : (tid < hp * hp ? 1 : 0);
+  // Q units (two rows rp, rp + hp of Q x the two columns of pivot k) belong to warps 1..3 only: they are rotated one
+  // round LATE, while warp 0 works out the rotations of the next round (Q does not enter the rotation angles)
+  const int nqu = hp * hp;                       // 256 (or 64 for a single-panel item)
+  int pend = 0, cur = 0;
+  const uchar2* prow = tab;
+  // Branch-free (an idle pivot carries the identity rotation cs = 1, s = 0, which leaves its operands bit-identical):
+  // the loads, the arithmetic and the stores of a thread's up to three units (which never overlap) interleave freely.
+  const int hsh = hp == U1_PB ? 4 : 3;            // hp = 1 << hsh
+  int qk[3], qrp[3];                               // pivot and row pair of this thread's three Q units (-1: none, warp-uniform)
+#pragma unroll
+  for (int x = 0; x < 3; ++x) {
+    const int u = tid - 32 + x * (SV_GROUP - 32);
+    qk[x] = (tid >= 32 && u < nqu) ? u >> hsh : -1;
+    qrp[x] = u & (hp - 1);
+  }
+  auto q_update = [&](const double4* Rp, const uchar2* rowp) {
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+      if (qk[x] >= 0) {   // warp-uniform
+        const Rot rj = load_rot(Rp, qk[x]);
+        const uchar2 vc = rowp[qk[x]];
+        cplx* cp = Qt + vc.x * SV_QLD + qrp[x];
+        cplx* cq = Qt + (vc.y & 0x7f) * SV_QLD + qrp[x];
+        cplx q00 = cp[0], q01 = cq[0], q10 = cp[hp], q11 = cq[hp];
+        rot_cols(q00, q01, rj); rot_cols(q10, q11, rj);
+        cplx* dp = (rj.flag & 2) ? cq : cp;
+        cplx* dq = (rj.flag & 2) ? cp : cq;
+        dp[0] = q00; dq[0] = q01; dp[hp] = q10; dq[hp] = q11;
+      }
+    }
+  };
   gsync(g);
+#ifdef EVD_CLK   // probe build only (_work/evd_bench.cu): cycles of the segments of a round, per warp
+  long long ck[5] = {0, 0, 0, 0, 0}, ct = clock64();
+#define EVD_TICK(k) do { const long long _n = clock64(); ck[k] += _n - ct; ct = _n; } while (0)
+#else
+#define EVD_TICK(k) do {} while (0)
+#endif
   for (int sw = 0; sw < inner_max; ++sw) {
     double mymax = 0.0;
     int sweep_any = 0;
     for (int t = 0; t < np2; ++t) {
-      const uchar2* row = tab + ((t + 1) % np2) * hp;   // pivots of this round
+      const uchar2* row = tab + ((t + 1) & (np2 - 1)) * hp;   // pivots of this round
+      double4* Rc = Rm + cur * U1_PB;
+      EVD_TICK(4);
       int rot = 0;
       if (tid < hp) {
         const uchar2 pv = row[tid];
         const int p = pv.x, q = pv.y & 0x7f;
         const double a = H[p * SV_HLD + p].x, b = H[q * SV_HLD + q].x;
         const cplx gg = H[p * SV_HLD + q];
-        const double g2 = gg.x * gg.x + gg.y * gg.y, ab = a * b;
+        const double g2 = fma(gg.x, gg.x, gg.y * gg.y), ab = a * b;
         double4 out = make_double4(1.0, 0.0, 0.0, 0.0);
         if (!(pv.y & 0x80) && ab > 0.0 && g2 > tol2 * ab && g2 > 1e-290) {
           rot = 1;
           mymax = fmax(mymax, g2 * rcp_approx(ab));
-          const double iag = rsqrt_approx(g2);                 // ~ 1/|g|
-          const double zeta = 0.5 * (b - a) * iag;
-          const double z1 = fma(zeta, zeta, 1.0);
-          const double tt = copysign(rcp_approx(fabs(zeta) + z1 * rsqrt_approx(z1)), zeta);
-          const double ti = tt * iag;
-          const double tx = ti * gg.x, ty = ti * gg.y;         // tau
-          const double n2 = fma(tx, tx, fma(ty, ty, 1.0));
-          double cs = rsqrt_approx(n2);                        // two Newton steps: full precision
-          cs = fma(0.5 * cs, fma(-n2 * cs, cs, 1.0), cs);
-          cs = fma(0.5 * cs, fma(-n2 * cs, cs, 1.0), cs);
-          const double sr = cs * tx, si = cs * ty;
+          // The rotation only has to shrink the off-diagonal entry (the iteration is self-correcting), so its angle is
+          // worked out in SINGLE precision - short latencies, and not on the FP64 pipe the DMMA streams of the other CTAs
+          // keep busy.  With d = (b - a)/2 and r = sqrt(d^2 + |g|^2) the small-angle Jacobi rotation has
+          //   cos^2 = 1/2 + |d|/(2r),   s = sign(d) g / (2 r cos)      (t = sign(zeta)/(|zeta| + sqrt(1 + zeta^2)), zeta = d/|g|)
+          // two MUFU rsqrt and a few FP32 operations.  g and d are first scaled by the power of two that brings the larger
+          // component of g to [1, 2) (exact).  Where |d| > 1e15 |g| (d^2 would leave the single-precision range) the
+          // small-angle limit cos = 1, s = g / (b - a) is exact to 1e-30.
+          const int ex = (__double2hiint(gg.x) >> 20) & 0x7ff, ey = (__double2hiint(gg.y) >> 20) & 0x7ff;
+          const double sc = __hiloint2double((2046 - min(max(ex, ey), 2045)) << 20, 0);
+          const float gxf = (float)(gg.x * sc), gyf = (float)(gg.y * sc);
+          const float dh = (float)((b - a) * (0.5 * sc));
+          double c0, s0x, s0y;
+          if (fabsf(dh) <= 1e15f) {
+            const float ir = rsqrtf(fmaf(dh, dh, fmaf(gxf, gxf, gyf * gyf)));
+            const float c2f = fmaf(0.5f * fabsf(dh), ir, 0.5f);
+            const float icf = rsqrtf(c2f);
+            const float kf = copysignf(0.5f * ir * icf, dh);
+            c0 = (double)(c2f * icf); s0x = (double)(kf * gxf); s0y = (double)(kf * gyf);
+          } else {
+            const double ri = rcp_approx(b - a);
+            c0 = 1.0; s0x = gg.x * ri; s0y = gg.y * ri;
+          }
+          // (cs, s) normalised in full precision: the rotation is unitary to rounding whatever the single-precision angle
+          // is.  c^2 + |s|^2 = 1 + O(1e-6), so two Newton steps from 1 give 1/sqrt to ~1e-24.
+          const double n2 = fma(c0, c0, fma(s0x, s0x, s0y * s0y));
+          double y = fma(-0.5, n2, 1.5);
+          y = y * fma(-0.5 * n2, y * y, 1.5);
+          const double cs = c0 * y, sr = s0x * y, si = s0y * y;
           // the pivot block after the rotation, in closed form (x' = cs x - conj(s) y, y' = s x + cs y):
           //   a' = cs^2 a + |s|^2 b - 2 cs Re(conj(s) g),  b' = |s|^2 a + cs^2 b + 2 cs Re(conj(s) g),
           //   g' = x'^H y' = cs s (a - b) + cs^2 g - s^2 conj(g)
@@ -304,10 +360,13 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
             H[p * SV_HLD + q] = make_double2(gnx, gny); H[q * SV_HLD + p] = make_double2(gnx, -gny);
           }
         }
-        Rm[tid] = out;
+        Rc[tid] = out;
       }
-      // this thread's H unit is loaded while warp 0 works out the rotations (the rotation threads only rewrite their
-      // own pivot blocks, never an off-diagonal unit)
+      EVD_TICK(0);
+      // ... while warps 1..3 catch up on Q with the rotations of the previous round
+      if (pend && tid >= 32) q_update(Rm + (cur ^ 1) * U1_PB, prow);
+      // this thread's H unit is loaded before the barrier (the rotation threads only rewrite their own pivot blocks,
+      // never an off-diagonal unit)
       int pi = 0, qi = 0, pj = 0, qj = 0;
       cplx b00, b01, b10, b11;
       if (uki >= 0) {
@@ -315,39 +374,25 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
         pi = vi.x; qi = vi.y & 0x7f; pj = vj.x; qj = vj.y & 0x7f;
         b00 = H[pi * SV_HLD + pj]; b01 = H[pi * SV_HLD + qj]; b10 = H[qi * SV_HLD + pj]; b11 = H[qi * SV_HLD + qj];
       }
+      EVD_TICK(1);
       const int any = gsync_or(g, rot);
+      EVD_TICK(2);
+      pend = any; prow = row; cur ^= 1;
       if (any) {  // uniform
         sweep_any = 1;
         if (uki >= 0) {
-          const Rot ri = load_rot(Rm, uki), rj = load_rot(Rm, ukj);
-          if (ri.flag | rj.flag) {
-            if (rj.flag) { rot_cols(b00, b01, rj); rot_cols(b10, b11, rj); }
-            if (ri.flag) { rot_rows(b00, b10, ri); rot_rows(b01, b11, ri); }
-            // exchanges are applied to the destinations
-            const int dpi = (ri.flag & 2) ? qi : pi, dqi = (ri.flag & 2) ? pi : qi;
-            const int dpj = (rj.flag & 2) ? qj : pj, dqj = (rj.flag & 2) ? pj : qj;
-            H[dpi * SV_HLD + dpj] = b00; H[dpi * SV_HLD + dqj] = b01; H[dqi * SV_HLD + dpj] = b10; H[dqi * SV_HLD + dqj] = b11;
-            H[dpj * SV_HLD + dpi] = make_double2(b00.x, -b00.y); H[dqj * SV_HLD + dpi] = make_double2(b01.x, -b01.y);
-            H[dpj * SV_HLD + dqi] = make_double2(b10.x, -b10.y); H[dqj * SV_HLD + dqi] = make_double2(b11.x, -b11.y);
-          }
+          // branch-free: an idle pivot carries the identity rotation, which leaves the unit bit-identical
+          const Rot ri = load_rot(Rc, uki), rj = load_rot(Rc, ukj);
+          rot_cols(b00, b01, rj); rot_cols(b10, b11, rj);
+          rot_rows(b00, b10, ri); rot_rows(b01, b11, ri);
+          // exchanges are applied to the destinations
+          const int dpi = (ri.flag & 2) ? qi : pi, dqi = (ri.flag & 2) ? pi : qi;
+          const int dpj = (rj.flag & 2) ? qj : pj, dqj = (rj.flag & 2) ? pj : qj;
+          H[dpi * SV_HLD + dpj] = b00; H[dpi * SV_HLD + dqj] = b01; H[dqi * SV_HLD + dpj] = b10; H[dqi * SV_HLD + dqj] = b11;
+          H[dpj * SV_HLD + dpi] = make_double2(b00.x, -b00.y); H[dqj * SV_HLD + dpi] = make_double2(b01.x, -b01.y);
+          H[dpj * SV_HLD + dqi] = make_double2(b10.x, -b10.y); H[dqj * SV_HLD + dqi] = make_double2(b11.x, -b11.y);
         }
-#pragma unroll
-        for (int x = 0; x < 2; ++x) {
-          if (x < nq) {
-            const Rot rj = load_rot(Rm, kq0 + 8 * x);
-            if (rj.flag) {
-              const uchar2 vc = row[kq0 + 8 * x];
-              const int pc = vc.x, qc = vc.y & 0x7f;
-              cplx* cp = Qt + pc * SV_QLD + rp;
-              cplx* cq = Qt + qc * SV_QLD + rp;
-              cplx q00 = cp[0], q01 = cq[0], q10 = cp[hp], q11 = cq[hp];
-              rot_cols(q00, q01, rj); rot_cols(q10, q11, rj);
-              cplx* dp = (rj.flag & 2) ? cq : cp;
-              cplx* dq = (rj.flag & 2) ? cp : cq;
-              dp[0] = q00; dq[0] = q01; dp[hp] = q10; dq[hp] = q11;
-            }
-          }
-        }
+        EVD_TICK(3);
         gsync(g);
       }
     }
@@ -355,6 +400,11 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
     ++*inner;
     if (!gsync_or(g, mymax > SV_QUAD)) break;
   }
+  if (pend && tid >= 32) q_update(Rm + (cur ^ 1) * U1_PB, prow);
+  gsync(g);
+#ifdef EVD_CLK
+  if ((tid & 31) == 0) for (int k = 0; k < 5; ++k) atomicAdd((unsigned long long*)&evd_clk[(tid >> 5) * 5 + k], (unsigned long long)ck[k]);
+#endif
 }
 
 // ---- phase 3: [Pa Pb] <- [Pa Pb] Q over all mt rows.  Warp w owns tile column w (8 columns) and all row tiles
@@ -423,9 +473,9 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
   cplx* stages = reinterpret_cast<cplx*>(smraw + (size_t)g * SV_GROUP_BYTES);
   cplx* Hs = stages;                               // [32*33], aliased onto the ring (idle during the EVD)
   cplx* Qs = Hs + SV_W * SV_HLD;                   // [32*36], transposed
-  double4* Rm = reinterpret_cast<double4*>(Qs + SV_W * SV_QLD);   // [16] rotations of the current EVD round
-  uchar2* tab = reinterpret_cast<uchar2*>(Rm + U1_PB);             // [32][16] pivots of the modulus ordering
-  static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD) * 16 + U1_PB * 32 + SV_W * U1_PB * 2, "EVD buffers must fit the idle stages");
+  double4* Rm = reinterpret_cast<double4*>(Qs + SV_W * SV_QLD);   // [2][16] rotations of the current and the previous EVD round
+  uchar2* tab = reinterpret_cast<uchar2*>(Rm + 2 * U1_PB);         // [32][16] pivots of the modulus ordering
+  static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD) * 16 + 2 * U1_PB * 32 + SV_W * U1_PB * 2, "EVD buffers must fit the idle stages");
   cg::grid_group grid = cg::this_grid();
   const int nblk = P.cnt[0], npair = P.cnt[1], maxP = P.cnt[3];
   const int R = max(maxP, 1);                      // rounds of one cycle of the largest sector (= a "sweep" of the trace)
