@@ -169,12 +169,8 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
     }
   }
   gsync(g);
-  // exact Hermitian symmetry from the upper triangle (the quick test and the rotations read p < q only)
-  for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
-    const int p = idx >> 5, q = idx & 31;
-    if (p > q) { const cplx v = Hs[q * SV_HLD + p]; Hs[p * SV_HLD + q] = make_double2(v.x, -v.y); }
-    else if (p == q) Hs[p * SV_HLD + p].y = 0.0;
-  }
+  // only the upper triangle of H is used from here on (the quick test and the EVD read row <= column)
+  if (gtid < SV_W) Hs[gtid * SV_HLD + gtid].y = 0.0;
   gsync(g);
 }
 
@@ -209,7 +205,15 @@ __device__ __forceinline__ void pivot(int t, int k, int np2, int* p, int* q) {
 #ifdef EVD_CLK
 __device__ long long evd_clk[20];
 #endif
-struct Rot { double cs, sr, si; int flag; };   // flag: 0 idle, 1 rotate, 3 rotate and exchange
+struct Rot { double cs, sr, si; int flag; };
+// H is kept as its upper triangle only (row <= column): entry (r, c) of the Hermitian matrix
+__device__ __forceinline__ cplx ldH(const cplx* H, int r, int c) {
+  const cplx v = H[min(r, c) * SV_HLD + max(r, c)];
+  return make_double2(v.x, r <= c ? v.y : -v.y);
+}
+__device__ __forceinline__ void stH(cplx* H, int r, int c, cplx v) {
+  H[min(r, c) * SV_HLD + max(r, c)] = make_double2(v.x, r <= c ? v.y : -v.y);
+}   // flag: 0 idle, 1 rotate, 3 rotate and exchange
 __device__ __forceinline__ Rot load_rot(const double4* Rm, int k) {
   const double4 v = Rm[k];
   Rot r; r.cs = v.x; r.sr = v.y; r.si = v.z; r.flag = (int)v.w;
@@ -307,7 +311,7 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
         const uchar2 pv = row[tid];
         const int p = pv.x, q = pv.y & 0x7f;
         const double a = H[p * SV_HLD + p].x, b = H[q * SV_HLD + q].x;
-        const cplx gg = H[p * SV_HLD + q];
+        const cplx gg = ldH(H, p, q);
         const double g2 = fma(gg.x, gg.x, gg.y * gg.y), ab = a * b;
         double4 out = make_double4(1.0, 0.0, 0.0, 0.0);
         if (!(pv.y & 0x80) && ab > 0.0 && g2 > tol2 * ab && g2 > 1e-290) {
@@ -352,13 +356,8 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
           const double gny = fma(cs * si, a - b, fma(c2, gg.y, -(s2i * gg.x - s2r * gg.y)));
           const bool swp = (p < q) ? (an < bn) : (bn < an);
           out = make_double4(cs, sr, si, swp ? 3.0 : 1.0);
-          if (swp) {
-            H[p * SV_HLD + p] = make_double2(bn, 0.0); H[q * SV_HLD + q] = make_double2(an, 0.0);
-            H[p * SV_HLD + q] = make_double2(gnx, -gny); H[q * SV_HLD + p] = make_double2(gnx, gny);
-          } else {
-            H[p * SV_HLD + p] = make_double2(an, 0.0); H[q * SV_HLD + q] = make_double2(bn, 0.0);
-            H[p * SV_HLD + q] = make_double2(gnx, gny); H[q * SV_HLD + p] = make_double2(gnx, -gny);
-          }
+          H[p * SV_HLD + p] = make_double2(swp ? bn : an, 0.0); H[q * SV_HLD + q] = make_double2(swp ? an : bn, 0.0);
+          stH(H, p, q, make_double2(gnx, swp ? -gny : gny));
         }
         Rc[tid] = out;
       }
@@ -372,7 +371,7 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
       if (uki >= 0) {
         const uchar2 vi = row[uki], vj = row[ukj];
         pi = vi.x; qi = vi.y & 0x7f; pj = vj.x; qj = vj.y & 0x7f;
-        b00 = H[pi * SV_HLD + pj]; b01 = H[pi * SV_HLD + qj]; b10 = H[qi * SV_HLD + pj]; b11 = H[qi * SV_HLD + qj];
+        b00 = ldH(H, pi, pj); b01 = ldH(H, pi, qj); b10 = ldH(H, qi, pj); b11 = ldH(H, qi, qj);
       }
       EVD_TICK(1);
       const int any = gsync_or(g, rot);
@@ -388,9 +387,7 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
           // exchanges are applied to the destinations
           const int dpi = (ri.flag & 2) ? qi : pi, dqi = (ri.flag & 2) ? pi : qi;
           const int dpj = (rj.flag & 2) ? qj : pj, dqj = (rj.flag & 2) ? pj : qj;
-          H[dpi * SV_HLD + dpj] = b00; H[dpi * SV_HLD + dqj] = b01; H[dqi * SV_HLD + dpj] = b10; H[dqi * SV_HLD + dqj] = b11;
-          H[dpj * SV_HLD + dpi] = make_double2(b00.x, -b00.y); H[dqj * SV_HLD + dpi] = make_double2(b01.x, -b01.y);
-          H[dpj * SV_HLD + dqi] = make_double2(b10.x, -b10.y); H[dqj * SV_HLD + dqi] = make_double2(b11.x, -b11.y);
+          stH(H, dpi, dpj, b00); stH(H, dpi, dqj, b01); stH(H, dqi, dpj, b10); stH(H, dqi, dqj, b11);
         }
         EVD_TICK(3);
         gsync(g);
