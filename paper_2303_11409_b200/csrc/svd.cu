@@ -87,23 +87,40 @@ struct Item {
 };
 
 // Stage rows [row0, row0 + SV_R) x the 32 columns of the item into shared memory (column-major, leading dimension ld);
-// rows >= rowlim and absent columns are zero-filled.
-__device__ __forceinline__ void load_chunk(cplx* st, int ld, const Item& I, int row0, int rowlim, int gtid) {
+// rows >= rowlim and absent columns are zero-filled.  Thread (r = gtid % 32, it) copies row row0 + r of the columns
+// j = gtid / 32 + 4 it; their addresses are worked out once per item (Loader), a chunk only adds its row offset.
+struct Loader {
+  const cplx* src[SV_W * SV_R / SV_GROUP];   // row r of column j (item's W if the column is absent: never read, 0 bytes copied)
+  unsigned ok;                                // bit it: column present
+};
+__device__ __forceinline__ Loader make_loader(const Item& I, int gtid) {
+  Loader L;
+  L.ok = 0;
   const int r = gtid & (SV_R - 1);
-  const bool rok = row0 + r < rowlim;
 #pragma unroll
   for (int it = 0; it < SV_W * SV_R / SV_GROUP; ++it) {
     const int j = gtid / SV_R + it * (SV_GROUP / SV_R);
-    const bool ok = rok && (j < U1_PB ? j < I.na : j - U1_PB < I.nb);
-    const cplx* src = ok ? I.W + (long long)I.col[j] * I.mt + row0 + r : I.W;
-    cp_async16(st + j * ld + r, src, ok ? 16 : 0);
+    const bool ok = j < U1_PB ? j < I.na : j - U1_PB < I.nb;
+    L.src[it] = ok ? I.W + (long long)I.col[j] * I.mt + r : I.W;
+    L.ok |= ok ? (1u << it) : 0u;
+  }
+  return L;
+}
+__device__ __forceinline__ void load_chunk(cplx* st, int ld, const Loader& L, int row0, int rowlim, int gtid) {
+  const int r = gtid & (SV_R - 1);
+  const bool rok = row0 + r < rowlim;
+  cplx* dst = st + (gtid / SV_R) * ld + r;
+#pragma unroll
+  for (int it = 0; it < SV_W * SV_R / SV_GROUP; ++it) {
+    const bool ok = rok && ((L.ok >> it) & 1u);
+    cp_async16(dst + it * (SV_GROUP / SV_R) * ld, ok ? L.src[it] + row0 : L.src[it], ok ? 16 : 0);
   }
 }
 
 // ---- phase 1: H = P^H P over rows [0, m).  H is Hermitian: only the 10 tiles (8 x 8 each) of the upper triangle of
 // the 4 x 4 tile grid are computed, 3 + 3 + 2 + 2 per warp: warp 0 (0,0) (0,1) (0,2); warp 1 (3,0) (3,1) (3,2), stored
 // as the conjugate transposes (0,3) (1,3) (2,3); warp 2 (1,1) (1,2); warp 3 (2,2) (3,3).
-__device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I, int g, int gtid) {
+__device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I, const Loader& L, int g, int gtid) {
   const int lane = gtid & 31, warp = gtid >> 5;
   const int lr = lane >> 2, lk = lane & 3;
   // tile slots of this warp: (ta[u], tb[u]), u < nt
@@ -121,14 +138,14 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
   const int nch = (I.m + SV_R - 1) / SV_R;
 #pragma unroll
   for (int p = 0; p < SV_NSTAGE - 1; ++p) {
-    if (p < nch) load_chunk(stages + p * SV_STAGE, SV_LDG, I, p * SV_R, I.m, gtid);
+    if (p < nch) load_chunk(stages + p * SV_STAGE, SV_LDG, L, p * SV_R, I.m, gtid);
     cp_async_commit();
   }
   for (int c = 0; c < nch; ++c) {
     cp_async_wait<SV_NSTAGE - 2>();
     gsync(g);  // chunk c has landed for everybody, and everybody is done with chunk c - 1: its stage may be refilled
     if (c + SV_NSTAGE - 1 < nch)
-      load_chunk(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDG, I, (c + SV_NSTAGE - 1) * SV_R, I.m, gtid);
+      load_chunk(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDG, L, (c + SV_NSTAGE - 1) * SV_R, I.m, gtid);
     cp_async_commit();
     const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE + lr * SV_LDG + lk;
     const int rows = min(SV_R, I.m - c * SV_R);
@@ -406,7 +423,7 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
 
 // ---- phase 3: [Pa Pb] <- [Pa Pb] Q over all mt rows.  Warp w owns tile column w (8 columns) and all row tiles
 // of each 32-row chunk; its 32 x 8 slice of Q lives in registers as 8 B fragments.
-__device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const Item& I, int g, int gtid) {
+__device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const Item& I, const Loader& L, int g, int gtid) {
   const int lane = gtid & 31, warp = gtid >> 5;
   const int tj = warp;
   const int lr = lane >> 2, lk = lane & 3;
@@ -429,14 +446,14 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
   const int nch = (I.mt + SV_R - 1) / SV_R;
 #pragma unroll
   for (int p = 0; p < SV_NSTAGE - 1; ++p) {
-    if (p < nch) load_chunk(stages + p * SV_STAGE, SV_LDU, I, p * SV_R, I.mt, gtid);
+    if (p < nch) load_chunk(stages + p * SV_STAGE, SV_LDU, L, p * SV_R, I.mt, gtid);
     cp_async_commit();
   }
   for (int c = 0; c < nch; ++c) {
     cp_async_wait<SV_NSTAGE - 2>();
     gsync(g);  // chunk c has landed for everybody, and everybody is done with chunk c - 1: its stage may be refilled
     if (c + SV_NSTAGE - 1 < nch)
-      load_chunk(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDU, I, (c + SV_NSTAGE - 1) * SV_R, I.mt, gtid);
+      load_chunk(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDU, L, (c + SV_NSTAGE - 1) * SV_R, I.mt, gtid);
     cp_async_commit();
     const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE;
     const int row0 = c * SV_R;
@@ -541,6 +558,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
         I.tol2 = tol * tol;
       }
       int todo = 0, big = 0;
+      Loader L;
       worked += have ? 1 : 0;
       if (have) {
         // logical -> physical columns: the order of the initial column norms (descending), so that the sweeps start
@@ -553,7 +571,8 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
         I.col = s_col[g];
         gsync(g);
         SV_TICK(0);
-        gram_phase(stages, Hs, I, g, gtid);
+        L = make_loader(I, gtid);
+        gram_phase(stages, Hs, I, L, g, gtid);
         SV_TICK(1);
         // quick test, same entries and arithmetic as the rotations: anything to do?
         for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
@@ -581,7 +600,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
       __syncthreads();
       SV_TICK(2);
       if (todo) {
-        update_phase(stages, Qs, I, g, gtid);
+        update_phase(stages, Qs, I, L, g, gtid);
         if (gtid == 0) { n_rot += 1; n_inner += inner; }
       }
       SV_TICK(3);
