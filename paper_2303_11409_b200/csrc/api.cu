@@ -48,7 +48,7 @@ Sizes compute_sizes(int M, int d, int N, int chi) {
   for (int i = 0; i < 5; ++i) add((E + 1) * 4);                  // rows cols keep blk tmpa
   add((E + 1) * 8); add((E + 1) * 4);                            // goff svoff
   add((E * d * d + 1) * 4); add((2 * E + 1) * 4);                // t2pref t5pref
-  add(8 * 4); add(2 * E * 4); add((size_t)2 * z.Gmax * 8);  // cnt flags gate_w
+  add(8 * 4); add(3 * E * 4); add((size_t)2 * z.Gmax * 8);  // cnt flags gate_w
   add(U1_SCHED * 4);                                             // sched
   add((4 * U1_MAXSWEEP + 1) * 8);                                // trace
   for (int i = 0; i < 2; ++i) add((size_t)z.itemcap * 4);        // item lists
@@ -130,6 +130,7 @@ int check_device_flags(u1mps* h) {  // after a sync
   CK(cudaMemcpyAsync(err, h->S.err, sizeof(err), cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
   if (err[0] == U1_ERR_WORKSPACE) return U1MPS_ENOMEM;
+  if (err[0] == U1_ERR_SCHED) return U1MPS_ECUDA;
   if (err[2] > 0) return U1MPS_ENOCONV;
   return U1MPS_OK;
 }
@@ -250,7 +251,7 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
   P.blk = A.take<int>(E + 1); P.tmpa = A.take<int>(E + 1);
   P.goff = A.take<long long>(E + 1); P.svoff = A.take<int>(E + 1);
   P.t2pref = A.take<int>(E * d * d + 1); P.t5pref = A.take<int>(2 * E + 1);
-  P.cnt = A.take<int>(8); P.flags = A.take<int>(2 * E); P.gate_w = A.take<double>((size_t)2 * z.Gmax);
+  P.cnt = A.take<int>(8); P.flags = A.take<int>(3 * E); P.gate_w = A.take<double>((size_t)2 * z.Gmax);
   P.sched = A.take<int>(U1_SCHED);
   P.trace = A.take<long long>(4 * U1_MAXSWEEP + 1);
   P.pitem_e = A.take<int>(z.itemcap); P.pitem_k = A.take<int>(z.itemcap);

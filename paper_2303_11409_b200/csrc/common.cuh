@@ -10,6 +10,7 @@ typedef double2 cplx;  // complex128, interleaved (x = re, y = im), 16-byte alig
 #define U1_MAXSWEEP 30     // Jacobi (outer) sweep limit
 #define U1_PB 16           // columns per Jacobi panel: a pair item orthogonalises 2*U1_PB = 32 columns
 #define U1_ERR_WORKSPACE 1 // device error flag: plan does not fit the workspace
+#define U1_ERR_SCHED 2     // device error flag: an a3 work-queue dependency did not resolve (internal error)
 #define U1_SCHED 264       // entries of Plan::sched
 #define U1_SVD_THREADS 128 // 4 warps per pair item, 6 CTAs per SM
 #define U1MPS_SORT_MAX 4096 // largest sector the in-smem bitonic sort takes (= U1MPS_CHI_MAX)
@@ -44,7 +45,7 @@ struct Plan {
   int* tmpa;         // [G*NC+1] scratch: pair-item offset per entry
   int* cnt;          // [8] 0: #blk, 1: #pair items, 3: max panels (even), 4: a2 tiles, 5: a5 tiles, 7: a4 CTA counter
   int* sched;        // [U1_SCHED] a3 scheduling state of one launch: work counters, tickets, CTA ranks per SM (svd.cu)
-  int* flags;        // [2*G*NC] a3 convergence stamps per entry: round after the last counting rotation, round found finished
+  int* flags;        // [3*G*NC] a3 per entry: round after the last counting rotation, round found finished, items completed
   long long* trace;  // [4*U1_MAXSWEEP] a3 trace of the last launch: per sweep end time (globaltimer ns), rotated items, inner sweeps, active sectors
   int* keep;         // [G*NC] kept singular values per entry (a4)
   int* perm;         // [pool] sorted position -> column index

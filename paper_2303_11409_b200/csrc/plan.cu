@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_kernel(DevState S, Plan P, 
     for (int k = 0; k < np; ++k) { P.pitem_e[off + k] = e; P.pitem_k[off + k] = k; }
   }
   atomicMax(&shmax, mymax);
-  for (int i = t; i < 2 * E; i += PLAN_THREADS) P.flags[i] = i < E ? 0 : 0x7fffffff;   // a3: last_rot[E], done_at[E]
+  for (int i = t; i < 3 * E; i += PLAN_THREADS) P.flags[i] = (i >= E && i < 2 * E) ? 0x7fffffff : 0;   // a3: last_rot[E], done_at[E], done_cnt[E]
   for (int i = t; i < 4 * U1_MAXSWEEP + 1; i += PLAN_THREADS) P.trace[i] = 0;
   for (int i = t; i < U1_SCHED; i += PLAN_THREADS) P.sched[i] = 0;
   __syncthreads();

@@ -19,12 +19,10 @@
 // spectrum from the top like a Gram-Schmidt pass, and needs about 2/3 of the sweeps of the round-robin tournament
 // on the Theta blocks of the workloads).  Convergence is decided on the device per sector (np consecutive rounds,
 // i.e. every panel pair once, without an off-diagonal Gram entry above the threshold), no host round trip.
-#include <cooperative_groups.h>
 #ifdef SV_PROFILE
 #include <cstdlib>
 #endif
 #include "common.cuh"
-namespace cg = cooperative_groups;
 
 #define SV_W 32                      // columns of a pair item
 #define SV_R 32                      // rows per staged chunk
@@ -37,7 +35,9 @@ namespace cg = cooperative_groups;
 #ifndef SV_ITEMS_PER_CTA
 #define SV_ITEMS_PER_CTA 4           // a3 throttle: items per active CTA and round below which fewer CTAs per SM are used
 #endif
+#ifndef SV_NSTAGE
 #define SV_NSTAGE 3                  // cp.async ring depth: chunks c + 1 and c + 2 are in flight while chunk c is consumed
+#endif
 #define SV_HLD 33                    // leading dimension of the 32 x 32 Gram matrix (row-major)
 static_assert(U1_MAXSWEEP == 30, "keep U1MPS_MAXSWEEP of include/u1mps.h in step");
 #define SV_QLD 36                    // leading dimension of the transposed eigenvector matrix Qt (4 mod 8: B fragments)
@@ -49,8 +49,10 @@ static_assert(U1_MAXSWEEP == 30, "keep U1MPS_MAXSWEEP of include/u1mps.h in step
 #define SV_QUAD 1e-4                 // no second inner sweep after one whose largest relative off-diagonal^2 was below this (measured best of 1e-14 .. 3e-1)
 #define SV_GROUP 128                 // threads per pair item (= one CTA: SV_NGROUP == 1; several groups per CTA were tried and dropped)
 #define SV_NGROUP (U1_SVD_THREADS / SV_GROUP)
+#ifndef SV_CTAS
 #define SV_CTAS 4                    // resident CTAs per SM the kernel is compiled for (registers <= 128: no spills with the
                                      // 3M accumulators; measured best of 3..6, profiles/r2_svd_tuning.md)
+#endif
 #define SV_GROUP_BYTES (SV_NSTAGE * SV_STAGE * 16)   // 36,864 B per group
 #define SV_SMEM_BYTES (SV_NGROUP * SV_GROUP_BYTES)
 
@@ -479,96 +481,133 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
   gsync(g);
 }
 
+__device__ __forceinline__ int ld_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+#define SV_SPIN_LIMIT (1u << 24)   // x >= 100 ns: a dependency that does not resolve within seconds is reported, not waited for
+
+// Work queue without grid-wide barriers.  Ticket T is item T % npair of round T / npair (the planner's list: the
+// (np + 1) / 2 pair slots of every sector, longest sectors first).  An item of round t may start once all items of ITS
+// sector of round t - 1 are done (a per-sector completion counter, release/acquire); items of different sectors never
+// wait for each other, so every sector advances at its own pace and no CTA idles at a barrier.  Tickets are handed out
+// in order and an item only waits for smaller tickets, whose holders are resident (cooperative launch): no deadlock.
 __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S, Plan P, int G, int inner_max, int sms) {
   extern __shared__ __align__(16) unsigned char smraw[];
-  __shared__ unsigned s_ticket;
-  __shared__ int s_col[SV_NGROUP][SV_W];
-  const int tid = threadIdx.x, g = tid / SV_GROUP, gtid = tid % SV_GROUP;
-  cplx* stages = reinterpret_cast<cplx*>(smraw + (size_t)g * SV_GROUP_BYTES);
+  __shared__ unsigned long long s_ticket;
+  __shared__ int s_go, s_fin, s_rank;
+  __shared__ int s_col[SV_W];
+  const int tid = threadIdx.x, g = 0, gtid = tid;
+  cplx* stages = reinterpret_cast<cplx*>(smraw);
   cplx* Hs = stages;                               // [32*33], aliased onto the ring (idle during the EVD)
   cplx* Qs = Hs + SV_W * SV_HLD;                   // [32*36], transposed
   double4* Rm = reinterpret_cast<double4*>(Qs + SV_W * SV_QLD);   // [2][16] rotations of the current and the previous EVD round
   uchar2* tab = reinterpret_cast<uchar2*>(Rm + 2 * U1_PB);         // [32][16] pivots of the modulus ordering
   static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD) * 16 + 2 * U1_PB * 32 + SV_W * U1_PB * 2, "EVD buffers must fit the idle stages");
-  cg::grid_group grid = cg::this_grid();
   const int nblk = P.cnt[0], npair = P.cnt[1], maxP = P.cnt[3];
   const int R = max(maxP, 1);                      // rounds of one cycle of the largest sector (= a "sweep" of the trace)
   const int E = G * S.NC;
   int* last_rot = P.flags;                         // [E] round after the last rotation outside the quadratic regime
   int* done_at = P.flags + E;                      // [E] round at which the sector was found converged (INT_MAX: not yet)
-  // Load-dependent throttle: a round hands its items to only as many CTAs per SM as the work warrants (the CTAs of an
-  // SM share the FP64 pipe, the shared-memory pipe and the issue slots: with few items per round every resident CTA beyond
-  // what is needed only slows the others down; measured in profiles/r2_svd_tuning.md).  Each CTA learns its rank on its SM
-  // once; the number of active ranks of the next round follows from the items that did work in this one.
-  int* sched = P.sched;   // [0..2] items that did work in round t (mod 3), [3..5] work-queue tickets (mod 3), [8 + smid] ranks
-  __shared__ int s_rank;
+  int* done_cnt = P.flags + 2 * E;                 // [E] items of the sector completed so far, over all rounds
+  // sched: [0..1] ticket (64 bit), [2] sectors finished, [3] CTAs that have left, [4] last round at which a sector finished,
+  // [5] abort, [8 + smid] CTA ranks.
+  // Load-dependent throttle: only as many CTAs per SM take items as the work warrants (the CTAs of an SM share the FP64
+  // pipe, the shared-memory pipe and the issue slots: with few items per round every resident CTA beyond what is needed
+  // only slows the others down; measured in profiles/r2_svd_tuning.md).
+  int* sched = P.sched;
   if (tid == 0) { unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid)); s_rank = atomicAdd(&sched[8 + (smid & 255)], 1); }
   __syncthreads();
-  const int rank = s_rank;
-  auto active_ranks = [&](int items) { return min(SV_CTAS, max(SV_MIN_ACTIVE, (items + SV_ITEMS_PER_CTA * sms - 1) / (SV_ITEMS_PER_CTA * sms))); };
-  int kact = active_ranks(npair);
+  const int kact = min(SV_CTAS, max(SV_MIN_ACTIVE, (npair + SV_ITEMS_PER_CTA * sms - 1) / (SV_ITEMS_PER_CTA * sms)));
   if (blockIdx.x == 0 && tid == 0) { long long t0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0)); P.trace[0] = t0; }
-  int tg = 0, n_rot = 0, n_inner = 0, ndone = 0;
 #ifdef SV_PROFILE   // debug build only: clock64 per phase, summed over the grid into the tail of the trace
   long long pc[6] = {0, 0, 0, 0, 0, 0}, pt = clock64();
 #define SV_TICK(k) do { const long long _n = clock64(); pc[k] += _n - pt; pt = _n; } while (0)
 #else
 #define SV_TICK(k) do {} while (0)
 #endif
-  for (; tg < U1_MAXSWEEP * R && nblk > 0; ++tg) {
-    unsigned* ticket = reinterpret_cast<unsigned*>(sched + 3 + tg % 3);
-    int worked = 0;
-    for (; rank < kact;) {
+  const unsigned long long total = (unsigned long long)npair * (unsigned long long)(U1_MAXSWEEP * R);
+  if (s_rank < kact && nblk > 0) {
+    for (;;) {
       __syncthreads();
-      if (tid == 0) s_ticket = atomicAdd(ticket, (unsigned)SV_NGROUP);
-      __syncthreads();
-      const unsigned it0 = s_ticket;
-      if (it0 >= (unsigned)npair) break;
-      const unsigned it = it0 + g;
-      bool have = it < (unsigned)npair;
-      Item I;
-      int e = 0;
-      if (have) {
-        e = P.pitem_e[it];
-        const int k = P.pitem_k[it];
-        const int r = P.rows[e], q = P.cols[e];
-        I.m = max(r, q);
-        const int n = min(r, q);
-        I.mt = I.m + n;
-        const int np = u1_ceil_div(n, U1_PB);
-        // the sector is finished once np consecutive rounds (= every panel pair once) needed no rotation outside the
-        // quadratic regime
-        if (tg - __ldcg(&last_rot[e]) >= np) {
-          have = false;
-          if (k == 0 && gtid == 0) atomicMin(&done_at[e], tg);
-        }
-        // modulus ordering (a pipelined cyclic-by-rows ordering): round tg pairs the panels with (i + j) mod np == rho
-        int pa = 0, pb = 1;
-        if (np > 1) {
-          const int rho = (tg + 1) % np;
-          const int na = (rho + 1) >> 1;
-          if (k < na) { pa = k; pb = rho - k; }
-          else { pa = rho + 1 + (k - na); pb = rho + np - pa; }
-          if (pa >= pb) have = false;
-        }
-        I.W = P.W + P.goff[e];
-        I.ca = pa * U1_PB; I.na = min(U1_PB, n - I.ca);
-        I.cb = pb * U1_PB; I.nb = pb < np ? min(U1_PB, n - I.cb) : 0;
-        const double tol = SV_TOLFAC * 1.1102230246251565e-16 * sqrt((double)I.m);
-        I.tol2 = tol * tol;
+      if (tid == 0) {
+        s_ticket = atomicAdd(reinterpret_cast<unsigned long long*>(sched), 1ull);
+        s_go = (ld_acquire(&sched[2]) < nblk && ld_acquire(&sched[5]) == 0) ? 1 : 0;
       }
+      __syncthreads();
+      const unsigned long long T = s_ticket;
+      if (T >= total || !s_go) break;
+      const int tg = (int)(T / (unsigned long long)npair);
+      const int it = (int)(T - (unsigned long long)tg * (unsigned long long)npair);
+      Item I;
+      const int e = P.pitem_e[it], k = P.pitem_k[it];
+      const int r = P.rows[e], q = P.cols[e], n = min(r, q);
+      I.m = max(r, q);
+      I.mt = I.m + n;
+      const int np = u1_ceil_div(n, U1_PB), slots = (np + 1) / 2;
+      // Thread 0 takes the scheduling decisions for the CTA (every value it reads may change under its eyes):
+      // s_go = 2: the sector was found finished in an earlier round - nothing to do (the item is still counted, so that
+      //           nobody waits for it); 1: go; 0: abort.  s_fin: the sector is finished as of this round.
+      SV_TICK(0);
+      if (tid == 0) {
+        int go = 1, fin = 0;
+        if (ld_acquire(&done_at[e]) < tg) {
+          go = 2;
+        } else {
+          // wait for the sector's items of the previous round
+          const int need = tg * slots;
+          unsigned spins = 0;
+          while (ld_acquire(&done_cnt[e]) < need) {
+            __nanosleep(100);
+            if (++spins > SV_SPIN_LIMIT || ld_acquire(&sched[5]) != 0) { go = 0; break; }
+          }
+          if (!go) { atomicExch(&sched[5], 1); atomicExch(S.err, U1_ERR_SCHED); }
+          // the sector is finished once np consecutive rounds (= every panel pair once) needed no rotation outside the
+          // quadratic regime (last_rot is final for the rounds before tg: they are complete; a stamp of this very
+          // round, tg + 1, reads as "not finished")
+          else if (tg - ld_acquire(&last_rot[e]) >= np) {
+            fin = 1;
+            if (k == 0 && atomicMin(&done_at[e], tg) == 0x7fffffff) {
+              atomicMax(&sched[4], tg);
+              __threadfence();
+              atomicAdd(&sched[2], 1);
+            }
+          }
+        }
+        if (go == 2) atomicAdd(&done_cnt[e], 1);
+        s_go = go; s_fin = fin;
+      }
+      __syncthreads();
+      if (s_go == 0) break;
+      if (s_go == 2) continue;
+      SV_TICK(4);
+      bool have = !s_fin;
+      // modulus ordering (a pipelined cyclic-by-rows ordering): round tg pairs the panels with (i + j) mod np == rho
+      int pa = 0, pb = 1;
+      if (np > 1) {
+        const int rho = (tg + 1) % np;
+        const int na = (rho + 1) >> 1;
+        if (k < na) { pa = k; pb = rho - k; }
+        else { pa = rho + 1 + (k - na); pb = rho + np - pa; }
+        if (pa >= pb) have = false;
+      }
+      I.W = P.W + P.goff[e];
+      I.ca = pa * U1_PB; I.na = min(U1_PB, n - I.ca);
+      I.cb = pb * U1_PB; I.nb = pb < np ? min(U1_PB, n - I.cb) : 0;
+      const double tol = SV_TOLFAC * 1.1102230246251565e-16 * sqrt((double)I.m);
+      I.tol2 = tol * tol;
       int todo = 0, big = 0;
       Loader L;
-      worked += have ? 1 : 0;
       if (have) {
         // logical -> physical columns: the order of the initial column norms (descending), so that the sweeps start
         // from a sorted matrix; the rotations keep exchanging logical columns, the map itself never changes
         if (gtid < SV_W) {
           const int j = gtid;
           const bool ok = j < U1_PB ? j < I.na : j - U1_PB < I.nb;
-          s_col[g][j] = ok ? P.perm[P.svoff[e] + (j < U1_PB ? I.ca + j : I.cb + j - U1_PB)] : 0;
+          s_col[j] = ok ? P.perm[P.svoff[e] + (j < U1_PB ? I.ca + j : I.cb + j - U1_PB)] : 0;
         }
-        I.col = s_col[g];
+        I.col = s_col;
         gsync(g);
         SV_TICK(0);
         L = make_loader(I, gtid);
@@ -599,51 +638,59 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
       if (todo) evd_phase(Hs, Qs, Rm, tab, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
       __syncthreads();
       SV_TICK(2);
-      if (todo) {
-        update_phase(stages, Qs, I, L, g, gtid);
-        if (gtid == 0) { n_rot += 1; n_inner += inner; }
-      }
+      if (todo) update_phase(stages, Qs, I, L, g, gtid);
       SV_TICK(3);
-    }
-    SV_TICK(0);
-    if (tid == 0 && worked) atomicAdd(&sched[tg % 3], worked);
-    grid.sync();
-    SV_TICK(4);
-    // the counters of round tg + 2 (last read after the grid sync of round tg - 1, which every CTA has left behind)
-    if (blockIdx.x == 0 && tid == 0) { sched[(tg + 2) % 3] = 0; sched[3 + (tg + 2) % 3] = 0; }
-    kact = active_ranks(__ldcg(&sched[tg % 3]));
-    // ---- convergence: sectors found finished up to this round (stamps of later rounds are ignored, so that every
-    // CTA takes the same decision)
-    int mine = 0;
-    for (int bi = tid; bi < nblk; bi += U1_SVD_THREADS) mine += (__ldcg(&done_at[P.blk[bi]]) <= tg) ? 1 : 0;
-    __shared__ int s_done;
-    if (tid == 0) s_done = 0;
-    __syncthreads();
-    if (mine) atomicAdd(&s_done, mine);
-    __syncthreads();
-    ndone = s_done;
-    const bool last = ndone == nblk;
-    if ((tg + 1) % R == 0 || last) {  // trace of this launch (u1mps_svd_trace), one entry per R rounds
-      const int sw = tg / R;
-      if (gtid == 0 && n_rot) {
-        atomicAdd((unsigned long long*)&P.trace[1 + U1_MAXSWEEP + sw], (unsigned long long)n_rot);
-        atomicAdd((unsigned long long*)&P.trace[1 + 2 * U1_MAXSWEEP + sw], (unsigned long long)n_inner);
-      }
-      n_rot = 0; n_inner = 0;
-      if (tid == 0 && blockIdx.x == 0) {
-        long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
-        P.trace[1 + sw] = t1;
-        P.trace[1 + 3 * U1_MAXSWEEP + sw] = nblk - ndone;
+      // done: publish (the update's stores and the stamp before the counter)
+      __syncthreads();
+      if (tid == 0) {
+        if (todo) {  // trace of this launch (u1mps_svd_trace), one entry per R rounds
+          const int sw = min(tg / R, U1_MAXSWEEP - 1);
+          long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+          atomicMax(&P.trace[1 + sw], t1);
+          atomicAdd((unsigned long long*)&P.trace[1 + U1_MAXSWEEP + sw], 1ull);
+          atomicAdd((unsigned long long*)&P.trace[1 + 2 * U1_MAXSWEEP + sw], (unsigned long long)inner);
+        }
+        __threadfence();
+        atomicAdd(&done_cnt[e], 1);
       }
     }
-    if (last) { ++tg; break; }
   }
+  SV_TICK(0);
 #ifdef SV_PROFILE
   if (tid == 0) for (int k = 0; k < 5; ++k) atomicAdd((unsigned long long*)&P.trace[1 + 3 * U1_MAXSWEEP + 20 + k], (unsigned long long)pc[k]);
 #endif
-  if (blockIdx.x == 0 && tid == 0) {
-    atomicMax(&S.err[1], (tg + R - 1) / R);
-    if (nblk > 0 && ndone < nblk) atomicAdd(&S.err[2], nblk - ndone);
+  // the last CTA to leave writes the statistics of the launch
+  __syncthreads();
+  if (tid == 0) { __threadfence(); s_go = (atomicAdd(&sched[3], 1) == (int)gridDim.x - 1) ? 1 : 0; }
+  __syncthreads();
+  if (s_go && nblk > 0) {
+    __threadfence();
+    const int fin = ld_acquire(&sched[2]);
+    const int rounds = fin == nblk ? ld_acquire(&sched[4]) + 1 : U1_MAXSWEEP * R;
+    const int nsw = min((rounds + R - 1) / R, U1_MAXSWEEP);
+#ifndef SV_PROFILE
+    // sectors not yet converged at the end of each sweep
+    for (int bi = tid; bi < nblk; bi += U1_SVD_THREADS) {
+      const int d = __ldcg(&done_at[P.blk[bi]]);
+      for (int sw = 0; sw < nsw; ++sw)
+        if (d > (sw + 1) * R - 1) atomicAdd((unsigned long long*)&P.trace[1 + 3 * U1_MAXSWEEP + sw], 1ull);
+    }
+#endif
+    if (tid == 0) {
+      atomicMax(&S.err[1], nsw);
+      if (fin < nblk && ld_acquire(&sched[5]) == 0) atomicAdd(&S.err[2], nblk - fin);
+      // end time of every sweep: the latest completion of one of its rotating items (sectors advance at their own
+      // pace, so sweeps overlap; a sweep without rotations ends with the launch), made monotone
+      long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+      long long prev = P.trace[0];
+      for (int sw = 0; sw < nsw; ++sw) {
+        long long v = P.trace[1 + sw];
+        if (v == 0) v = t1;
+        v = max(v, prev);
+        P.trace[1 + sw] = v;
+        prev = v;
+      }
+    }
   }
 }
 
