@@ -30,7 +30,7 @@
 #define SV_LDU 34                    // ... in the update phase: 2 mod 8 (both: conflict-free LDS.128 fragment loads)
 #define SV_STAGE (SV_W * SV_LDG)     // complex elements per stage
 #ifndef SV_MIN_ACTIVE
-#define SV_MIN_ACTIVE 2
+#define SV_MIN_ACTIVE 2                  // a3 throttle: CTAs per SM that take items however little work there is
 #endif
 #ifndef SV_ITEMS_PER_CTA
 #define SV_ITEMS_PER_CTA 4           // a3 throttle: items per active CTA and round below which fewer CTAs per SM are used
@@ -53,8 +53,9 @@ static_assert(U1_MAXSWEEP == 30, "keep U1MPS_MAXSWEEP of include/u1mps.h in step
 #define SV_CTAS 4                    // resident CTAs per SM the kernel is compiled for (registers <= 128: no spills with the
                                      // 3M accumulators; measured best of 3..6, profiles/r2_svd_tuning.md)
 #endif
-#define SV_GROUP_BYTES (SV_NSTAGE * SV_STAGE * 16)   // 36,864 B per group
-#define SV_SMEM_BYTES (SV_NGROUP * SV_GROUP_BYTES)
+#define SV_RING_BYTES (SV_NSTAGE * SV_STAGE * 16)
+#define SV_EVD_BYTES ((SV_W * SV_HLD + SV_W * SV_QLD) * 16 + 2 * U1_PB * 32 + SV_W * U1_PB * 2)   // H, Qt, rotations, pivot table
+#define SV_SMEM_BYTES (SV_RING_BYTES > SV_EVD_BYTES ? SV_RING_BYTES : SV_EVD_BYTES)   // the EVD buffers alias the idle ring
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -504,7 +505,6 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
   cplx* Qs = Hs + SV_W * SV_HLD;                   // [32*36], transposed
   double4* Rm = reinterpret_cast<double4*>(Qs + SV_W * SV_QLD);   // [2][16] rotations of the current and the previous EVD round
   uchar2* tab = reinterpret_cast<uchar2*>(Rm + 2 * U1_PB);         // [32][16] pivots of the modulus ordering
-  static_assert(SV_NSTAGE * SV_STAGE * 16 >= (SV_W * SV_HLD + SV_W * SV_QLD) * 16 + 2 * U1_PB * 32 + SV_W * U1_PB * 2, "EVD buffers must fit the idle stages");
   const int nblk = P.cnt[0], npair = P.cnt[1], maxP = P.cnt[3];
   const int R = max(maxP, 1);                      // rounds of one cycle of the largest sector (= a "sweep" of the trace)
   const int E = G * S.NC;

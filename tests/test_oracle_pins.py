@@ -382,3 +382,57 @@ def test_truncation_is_reported_and_state_stays_normalised():
     # canonical-form <n> is only approximate once truncation has broken canonicity (SURVEY §8(c) Readouts)
     assert abs(sum(st.expect_n(s) for s in range(w.M)) - w.N) < 2e-2
     assert abs(sum(st.expect_n_full(s) for s in range(w.M)) - w.N) < 1e-11
+
+
+# ------------------------------------------------------------------ P11: the order at the cut (readings S7, S8)
+def test_P11_tie_order_and_keep_at_least_one():
+    """DESIGN reading S8 (the paper is silent): ties at the chi-th value go to (sigma desc, c asc, j asc); reading S7:
+    at least one value is always kept.  Constructed exact ties: the hop / stay gate below splits |..10..> into two
+    charge sectors with bitwise equal singular values.  The expected kept set is worked out here from the dense Theta of
+    Eq.11 (one plain SVD per charge block cut out of the dense matrix by the occupations - not by the oracle's sector
+    code) with the rule written out again; a c-descending or j-descending tie-break fails."""
+    a = 0.7071067811865476
+    U = np.zeros((4, 4), dtype=np.complex128)
+    U[0, 0] = U[3, 3] = 1.0
+    U[1, 1] = U[1, 2] = U[2, 1] = a
+    U[2, 2] = -a
+    # two-site chain: Theta(c = 0) = [a], Theta(c = 1) = [a]
+    st = U1MPS.product_state(2, 2, 1, 4, [1, 0])
+    rec = st.apply_gate(0, U, chi=1, cutoff=1e-12, record=True)
+    assert rec.sigma[0][0] == rec.sigma[1][0] == a          # an exact tie
+    assert rec.keep == {0: 1, 1: 0} and st.sectors[1] == [0]
+    # keep at least one: a cutoff above every singular value keeps the first of the order, nothing else
+    st = U1MPS.product_state(2, 2, 1, 4, [1, 0])
+    rec = st.apply_gate(0, U, chi=4, cutoff=2.0, record=True)
+    assert rec.keep == {0: 1, 1: 0} and abs(st.lam[1][0][0] - 1.0) < 1e-15
+    # a chain where the tied sectors hold several values each: two hop / stay gates on |1010> make bond 2 carry the
+    # sectors c = 0, 1, 2; the middle gate then sees degenerate pairs across sectors
+    st = U1MPS.product_state(4, 2, 2, 16, [1, 0, 1, 0])
+    st.apply_gate(0, U, cutoff=1e-12)
+    st.apply_gate(2, U, cutoff=1e-12)
+    gams, lams = st.to_dense()
+    ref = st.copy()
+    for chi in (1, 2, 3):
+        t = ref.copy()
+        rec = t.apply_gate(1, U, chi=chi, cutoff=1e-12, record=True)
+        # dense Theta of Eq.11, rows (i, alpha), columns (j, gamma); charge of a column = charge of gamma + j
+        U4 = U.reshape(2, 2, 2, 2)
+        A = lams[1][None, :, None] * gams[1] * lams[2][None, None, :]
+        B = gams[2] * lams[3][None, None, :]
+        theta = np.einsum("xyij,iab,jbg->xayg", U4, A, B)
+        cR = np.concatenate([[c] * len(st.lam[3][c]) for c in st.sectors[3]])
+        pool = []
+        for c in range(0, 3):
+            cols = [(y, g_) for y in range(2) for g_ in range(len(cR)) if cR[g_] + y == c]
+            if not cols:
+                continue
+            blk = np.stack([theta[:, :, y, g_].reshape(-1) for y, g_ in cols], axis=1)
+            sv_ = np.linalg.svd(blk, compute_uv=False)
+            pool += [(float(x), c, j) for j, x in enumerate(sv_) if x > 1e-12]
+        order = sorted(pool, key=lambda p: (-p[0], p[1], p[2]))[:chi]
+        want = {}
+        for _, c, _ in order:
+            want[c] = want.get(c, 0) + 1
+        assert {c: k for c, k in rec.keep.items() if k > 0} == want, (chi, rec.keep, want)
+    sig = sorted((float(x), c) for c, v in rec.sigma.items() for x in v if x > 1e-12)
+    assert any(abs(x - y) == 0.0 and c1 != c2 for (x, c1), (y, c2) in zip(sig[:-1], sig[1:]))   # ties across sectors exist
