@@ -44,7 +44,7 @@ from paper_2303_11409_b200 import inputs  # noqa: E402  (seeded input generators
 # FP64 peak used as the "alu" roofline denominator: 148 SMs x 64 FP64 FMA/clk/SM x 2 flop
 # x 1.965 GHz (clocks.max.sm of MEASURED_PEAKS.json).  MEASURED_PEAKS.json has no FP64 entry; the probe result is in DESIGN.md.
 FP64_FMA_PER_CLK_PER_SM = 64
-SYNTH_R = {2: 9, 3: 11, 4: 13, 5: 21}   # number of charge sectors of a saturated bond (DESIGN.md §Input recipe)
+SYNTH_R = {1: 4, 2: 9, 3: 11, 4: 13, 5: 21}   # number of charge sectors of a saturated bond (DESIGN.md §Input recipe)
 
 
 def fp64_peak_tflops():
@@ -218,17 +218,6 @@ def memory_stages(prof, work, work_after, steps):
                            "bytes_per_step": by / steps, "ms_per_step": ms / steps}}
 
 
-def svd_traffic_bytes():
-    """DRAM bytes (read + write) of ONE a3 launch from the committed ncu --set full capture, or None."""
-    try:
-        import csv
-        with open(os.path.join(ROOT, "profiles", "svd_traffic.csv")) as f:
-            row = next(csv.DictReader(f))
-        return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
-    except Exception:
-        return None
-
-
 def run_reference(args, w):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -256,10 +245,154 @@ def run_reference(args, w):
 
 
 # ----------------------------------------------------------------------------- our arm
+def fp64_probe():
+    """Measured DFMA / DMMA throughput of this GPU (paper_2303_11409_b200/csrc/fp64_probe.cu, built by build())."""
+    exe = os.path.join(ROOT, "paper_2303_11409_b200", "fp64_probe")
+    try:
+        out = subprocess.run([exe], capture_output=True, text=True, timeout=60).stdout.strip().splitlines()[-1]
+        return json.loads(out)
+    except Exception as e:  # the probe is a report, not a dependency of the measurement
+        return {"error": f"{type(e).__name__}: {e}"}
+
+
+def readout_bytes(gpu, w):
+    """Algorithmic bytes of one a6 read-out of the whole chain: <n_k> reads every Gamma block with occupation >= 1 once
+    (16 B per element) and the lambda vectors of its two bonds; the entropies read every lambda once."""
+    tabs = [dict(gpu.bond_info(k)) for k in range(w.M + 1)]
+    by = 0
+    for s in range(w.M):
+        for cl, nl in tabs[s].items():
+            for i in range(1, w.d):
+                by += 16 * nl * tabs[s + 1].get(cl - i, 0)
+        by += 8 * (sum(tabs[s].values()) + sum(tabs[s + 1].values()))
+    by += 8 * sum(sum(t.values()) for t in tabs)
+    return by
+
+
+def measure(w, args, steps, warmup, prep_columns, with_e2e, rank, world, local, barrier):
+    """One workload on this rank's GPU: the config's own columns as preparation, then `steps` timed brick-wall layers."""
+    import torch
+    from paper_2303_11409_b200.binding import U1MPS, load_library
+    Gcol = w.M // 2
+    ws_gate = 2 * w.d * w.chi * w.chi * 16
+    need = load_library().u1mps_workspace_bytes(w.M, w.d, w.N, w.chi)
+    free, _ = torch.cuda.mem_get_info()
+    arena = min(need + Gcol * ws_gate, int(free * 0.8))
+    gpu = U1MPS(w.M, w.d, w.N, w.chi, arena_bytes=arena)
+    gpu.set_product_state(w.occ)
+
+    cols_per_layer = 2
+    n_prep = w.columns if prep_columns < 0 else prep_columns
+    n_total = n_prep + cols_per_layer * (warmup + steps) * (2 if with_e2e else 1) + cols_per_layer
+    host_cols = list(inputs.gate_columns(dataclasses.replace(w, columns=n_total)))
+    dev_cols = [(s, torch.from_numpy(u).cuda()) for s, u in host_cols]
+    pin_cols = [(s, torch.from_numpy(u).pin_memory()) for s, u in host_cols] if with_e2e else None
+    col = 0
+
+    # ---- preparation: the config's own trajectory (untimed for the metric; reported)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(n_prep):
+        gpu.apply_gate_column(dev_cols[col][0], dev_cols[col][1], cutoff=w.cutoff)
+        col += 1
+    e1.record()
+    torch.cuda.synchronize()
+    prep_ms = e0.elapsed_time(e1)
+    prep_gates = sum(len(host_cols[c][0]) for c in range(n_prep))
+    work = layer_work(gpu, w)
+    gates_per_step = sum(len(inputs.column_sites(w.M, t)) for t in (0, 1))
+
+    def layer(cols_src):
+        nonlocal col
+        for _ in range(cols_per_layer):
+            gpu.apply_gate_column(cols_src[col][0], cols_src[col][1], cutoff=w.cutoff)
+            col += 1
+
+    # ---- device-resident timed region
+    for _ in range(warmup):
+        layer(dev_cols)
+    sampler = ClockSampler(local) if (rank == 0 and with_e2e) else None
+    gpu.profile_enable(True)
+    l0 = gpu.launch_count()
+    barrier()
+    e0.record()
+    for _ in range(steps):
+        layer(dev_cols)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = gpu.launch_count() - l0
+    prof = gpu.profile_read()
+    clocks = sampler.stop() if sampler else None
+    work_after = layer_work(gpu, w)
+
+    # ---- end-to-end timed region: host gate buffers in, readouts out (per-kernel events stay on: a6 is timed here)
+    ms_e2e = None
+    a6 = None
+    n_k = gpu.expect_n_all()
+    ln = gpu.log_norm(allow_nonconverged=True)
+    if with_e2e:
+        for _ in range(min(warmup, 1)):
+            layer(pin_cols)
+            gpu.expect_n_all(); gpu.bond_entropy_all(); gpu.log_norm(allow_nonconverged=True)
+        gpu.profile_read()
+        barrier()
+        e0.record()
+        for _ in range(steps):
+            layer(pin_cols)
+            n_k = gpu.expect_n_all()
+            s_k = gpu.bond_entropy_all()
+            ln = gpu.log_norm(allow_nonconverged=True)
+        e1.record()
+        barrier()
+        ms_e2e = e0.elapsed_time(e1)
+        a6_ms, a6_n = gpu.profile_read()["a6_readout"]
+        a6 = {"ms_per_step": a6_ms / steps, "launches_per_step": a6_n / steps, "bytes_per_step": readout_bytes(gpu, w)}
+    gpu.profile_enable(False)
+    stats = gpu.last_stats()
+    res = {"w": w, "ms": ms, "ms_e2e": ms_e2e, "launches": launches, "prof": prof, "clocks": clocks, "work": work,
+           "work_after": work_after, "gates_per_step": gates_per_step, "prep_ms": prep_ms, "prep_gates": prep_gates,
+           "n_prep": n_prep, "stats": stats, "sum_n": float(np.sum(n_k)), "log_norm": ln, "a6": a6, "steps": steps}
+    gpu.close()
+    del gpu, dev_cols, pin_cols
+    torch.cuda.empty_cache()
+    return res
+
+
+def a3_roofline(res, peak):
+    """Useful FP64 rate of the a3 launches of a measurement against the FP64 peak."""
+    svd_ms, svd_n = res["prof"]["a3_svd"]
+    per_launch = 0.5 * (res["work"]["a3_flops"] + res["work_after"]["a3_flops"]) / 2   # per column = per launch
+    achieved = per_launch / (svd_ms / max(svd_n, 1) * 1e-3) / 1e12 if svd_ms > 0 else 0.0
+    return achieved, achieved / peak, svd_ms / max(svd_n, 1), svd_n
+
+
+def hbm_peak():
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        return None
+
+
+def svd_traffic_bytes(name):
+    """DRAM bytes (read + write) of ONE a3 launch from the committed ncu --set full capture of THIS workload, or None."""
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", f"svd_traffic_{name}.csv")) as f:
+            row = next(csv.DictReader(f))
+        return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
+    except Exception:
+        return None
+
+
+# per-workload side measurements of the default run: (prep columns, warm-up steps, timed steps, oracle gates)
+SIDE = {1: (-1, 3, 4, 64), 2: (-1, 3, 3, 32), 3: (-1, 3, 3, 24), 4: (-1, 3, 3, 8), 5: (12, 0, 1, 1)}
+
+
 def run_ours(args, w):
     import torch
     import torch.distributed as dist
-    from paper_2303_11409_b200.binding import U1MPS
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -275,101 +408,34 @@ def run_ours(args, w):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # arena: state + plan + workspace for a whole column of saturated gates
-    Gcol = w.M // 2
-    ws_gate = 2 * w.d * w.chi * w.chi * 16
-    from paper_2303_11409_b200.binding import load_library
-    need = load_library().u1mps_workspace_bytes(w.M, w.d, w.N, w.chi)
-    free, _ = torch.cuda.mem_get_info()
-    arena = min(need + Gcol * ws_gate, int(free * 0.8))
-    gpu = U1MPS(w.M, w.d, w.N, w.chi, arena_bytes=arena)
-    gpu.set_product_state(w.occ)
-
-    cols_per_layer = 2
-    n_prep = w.columns if args.prep_columns < 0 else args.prep_columns
-    n_total = n_prep + cols_per_layer * (args.warmup + args.steps) * 2 + cols_per_layer
-    host_cols = list(inputs.gate_columns(dataclasses.replace(w, columns=n_total)))
-    dev_cols = [(s, torch.from_numpy(u).cuda()) for s, u in host_cols]
-    pin_cols = []
-    for s, u in host_cols:
-        t = torch.from_numpy(u).pin_memory()
-        pin_cols.append((s, t))
-    col = 0
-
-    # ---- preparation: the config's own trajectory (untimed for the metric; reported)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(n_prep):
-        gpu.apply_gate_column(dev_cols[col][0], dev_cols[col][1], cutoff=w.cutoff)
-        col += 1
-    e1.record()
-    torch.cuda.synchronize()
-    prep_ms = e0.elapsed_time(e1)
-    prep_gates = sum(len(host_cols[c][0]) for c in range(n_prep))
-    stats_prep = gpu.last_stats()
-    work = layer_work(gpu, w)
-    gates_per_step = sum(len(inputs.column_sites(w.M, t)) for t in (0, 1))
-
-    def layer(cols_src):
-        nonlocal col
-        for _ in range(cols_per_layer):
-            gpu.apply_gate_column(cols_src[col][0], cols_src[col][1], cutoff=w.cutoff)
-            col += 1
-
-    # ---- device-resident timed region
-    for _ in range(args.warmup):
-        layer(dev_cols)
-    sampler = ClockSampler(local) if rank == 0 else None
-    gpu.profile_enable(True)
-    l0 = gpu.launch_count()
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        layer(dev_cols)
-    e1.record()
-    barrier()
-    ms = e0.elapsed_time(e1)
-    launches = gpu.launch_count() - l0
-    prof = gpu.profile_read()
-    gpu.profile_enable(False)
-    clocks = sampler.stop() if sampler else None
-    work_after = layer_work(gpu, w)
-
-    # ---- end-to-end timed region: host gate buffers in, readouts out
-    for _ in range(min(args.warmup, 1)):
-        layer(pin_cols)
-        gpu.expect_n_all(); gpu.bond_entropy_all(); gpu.log_norm()
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        layer(pin_cols)
-        n_k = gpu.expect_n_all()
-        s_k = gpu.bond_entropy_all()
-        ln = gpu.log_norm()
-    e1.record()
-    barrier()
-    ms_e2e = e0.elapsed_time(e1)
-    h2d = gates_per_step * (w.d ** 4) * 16 + gates_per_step * 4
-    d2h = (w.M + (w.M + 1) + 1) * 8 + 3 * 4
-    stats = gpu.last_stats()
-    total_n = float(np.sum(n_k))
-
-    ms, ms_e2e = dist_max([ms, ms_e2e], world, "cuda")
+    probe = fp64_probe() if rank == 0 else None
+    res = measure(w, args, args.steps, args.warmup, args.prep_columns, True, rank, world, local, barrier)
+    ms, ms_e2e = dist_max([res["ms"], res["ms_e2e"]], world, "cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
+    gates_per_step = res["gates_per_step"]
+    work, work_after, prof, stats = res["work"], res["work_after"], res["prof"], res["stats"]
     n_gates = args.steps * gates_per_step * world
     value = n_gates / (ms * 1e-3)
     e2e = n_gates / (ms_e2e * 1e-3)
-    svd_ms, svd_n = prof["a3_svd"]
+    h2d = gates_per_step * (w.d ** 4) * 16 + gates_per_step * 4
+    d2h = (w.M + (w.M + 1) + 1) * 8 + 3 * 4
     peak = fp64_peak_tflops()
-    a3_flops_launch = 0.5 * (work["a3_flops"] + work_after["a3_flops"]) / cols_per_layer   # per column = per launch
-    achieved = a3_flops_launch / (svd_ms / max(svd_n, 1) * 1e-3) / 1e12 if svd_ms > 0 else 0.0
+    achieved, frac, ms_launch, svd_n = a3_roofline(res, peak)
+    svd_ms = prof["a3_svd"][0]
     useful_flops_step = 0.5 * (work["a2_flops"] + work["a3_flops"] + work_after["a2_flops"] + work_after["a3_flops"])
     stage_ms = {k: round(v[0] / args.steps, 4) for k, v in prof.items()}
+    stage_ms["a6_readout"] = round(res["a6"]["ms_per_step"], 4)   # timed in the end-to-end region (the device-resident one reads nothing)
+    mem = memory_stages(prof, work, work_after, args.steps) or {}
+    hbm = hbm_peak()
+    if res["a6"]["ms_per_step"] > 0:
+        gbs = res["a6"]["bytes_per_step"] / (res["a6"]["ms_per_step"] * 1e-3) / 1e9
+        mem["a6_readout"] = {"achieved": gbs, "unit": "GB/s", "peak": hbm, "frac": (gbs / hbm) if hbm else None,
+                             "bytes_per_step": res["a6"]["bytes_per_step"], "ms_per_step": res["a6"]["ms_per_step"],
+                             "note": "<n_k> of all sites + all bond entropies once per step, CUDA-event time of the a6 kernels"}
 
     # ---- the oracle timed beside it (rank 0, N = 1 only)
     cpu = None
@@ -379,13 +445,42 @@ def run_ours(args, w):
                "sample": f"{args.cpu_gates} gates on seeded synthetic saturated-bond states (d={w.d}, chi={w.chi}, "
                          f"{sample_profile(w)}), {secs:.1f} s of numpy/LAPACK work"}
 
+    # ---- the other workloads of BASELINE.json, shorter (rank 0, N = 1 only): gates/s, a3 roofline fraction, oracle beside it
+    per_workload = None
+    if world == 1 and not args.no_per_workload:
+        per_workload = {}
+        for idx in sorted(inputs.WORKLOADS):
+            wi = inputs.WORKLOADS[idx]
+            if idx == w.index:
+                per_workload[wi.name] = {"gates_per_s": value, "a3_frac_of_fp64_peak": frac, "svd_sweeps_max": stats["sweeps"],
+                                         "cpu_baseline_gates_per_s": cpu["value"] if cpu else None, "note": "the headline measurement above"}
+                continue
+            prep, wu, st_, og = SIDE[idx]
+            r = measure(wi, args, st_, wu, prep, False, 0, 1, local, barrier)
+            ach, fr, msl, _ = a3_roofline(r, peak)
+            entry = {"gates_per_s": st_ * r["gates_per_step"] / (r["ms"] * 1e-3), "ms_per_step": r["ms"] / st_, "steps": st_, "warmup": wu,
+                     "prep_columns": r["n_prep"], "trajectory_gates_per_s": r["prep_gates"] / (r["prep_ms"] * 1e-3) if r["prep_ms"] > 0 else None,
+                     "a3_useful_tflops": ach, "a3_frac_of_fp64_peak": fr, "a3_ms_per_launch": msl,
+                     "a3_share_of_step": r["prof"]["a3_svd"][0] / r["ms"] if r["ms"] > 0 else None,
+                     "svd_sweeps_max": r["stats"]["sweeps"], "svd_converged": r["stats"]["converged"],
+                     "bond_dim_max": r["work"]["bond_dim_max"], "max_block": r["work"]["max_block"], "sum_n": r["sum_n"]}
+            if idx == 5:
+                entry["note"] = ("bounded: state after the first 12 of the config's 100 columns (47 of 101 bonds at chi = 4096), "
+                                 "one timed layer, no separate warm-up (the preparation columns are the warm-up)")
+            if not args.no_cpu_baseline:
+                rate, secs, cores = oracle_sample(wi, og)
+                entry["cpu_baseline_gates_per_s"] = rate
+                entry["cpu_baseline_sample"] = f"{og} synthetic saturated-bond gates, {secs:.1f} s on {cores} cores"
+            per_workload[wi.name] = entry
+
+    traffic = svd_traffic_bytes(w.name)
     out = {
         "metric": "two-site U(1) gate updates/sec", "value": value, "unit": "gates/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "c128", "data": "synthetic",
         "config": {"workload": w.name, "M": w.M, "d": w.d, "N": w.N, "chi": w.chi, "cutoff": w.cutoff,
                    "step": f"one brick-wall layer ({gates_per_step} gates, 2 launches of every kernel) on the state after "
-                           f"{n_prep} columns of the config's trajectory",
+                           f"{res['n_prep']} columns of the config's trajectory",
                    "l2": "state touched per step exceeds L2 (inputs larger than L2, no flush)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "bond_dim_max": work["bond_dim_max"], "bond_dim_median": work["bond_dim_median"],
@@ -393,27 +488,31 @@ def run_ours(args, w):
                    "max_block": work["max_block"]},
         "e2e": {"value": e2e, "unit": "gates/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": ms_e2e / args.steps},
-        "gpu_launches": int(launches),
-        "clocks": clocks,
+        "gpu_launches": int(res["launches"]),
+        "clocks": res["clocks"],
         "roofline": {"kernel": "svd_kernel (a3)", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                     "frac": achieved / peak, "traffic": svd_traffic_bytes(),
-                     "peak_source": "derived: 148 SMs x 64 FP64 FMA/clk x 2 x sm_max_mhz (no FP64 entry in MEASURED_PEAKS.json; "
-                                    "the round-1 probe measured 36.8 DFMA / 37.06 DMMA TFLOP/s, DESIGN.md section 6)",
-                     "traffic_source": "profiles/svd_traffic.csv (ncu --set full, one launch of the same workload)",
+                     "frac": frac, "traffic": traffic,
+                     "peak_source": "derived: 148 SMs x 64 FP64 FMA/clk x 2 x sm_max_mhz (no FP64 entry in MEASURED_PEAKS.json); "
+                                    "measured in this run by paper_2303_11409_b200/csrc/fp64_probe.cu: see peak_probe",
+                     "peak_probe": probe,
+                     "traffic_source": (f"profiles/svd_traffic_{w.name}.csv (ncu --set full, one launch of this workload)"
+                                        if traffic is not None else "no committed ncu capture of this workload"),
                      "flops": "useful SVD flops 4*min(14mn^2+8n^3, 6mn^2+20n^3) per block (SURVEY §8(d))",
-                     "ms_per_launch": svd_ms / max(svd_n, 1), "launches": svd_n,
+                     "ms_per_launch": ms_launch, "launches": svd_n,
                      "share_of_step": svd_ms / ms if ms > 0 else None},
         "useful_gflops": useful_flops_step * args.steps * world / (ms * 1e-3) / 1e9,
-        "memory_bound_stages": memory_stages(prof, work, work_after, args.steps),
+        "memory_bound_stages": mem or None,
         "a2_contract": {"useful_tflops": (0.5 * (work["a2_flops"] + work_after["a2_flops"]) * args.steps
                                           / (prof["a2_contract"][0] * 1e-3) / 1e12) if prof["a2_contract"][0] > 0 else None,
                         "note": "minimum-form flops 8 nL nC nR per (c_l, c', c_r) triple / summed CUDA-event time of contract_kernel"},
         "useful_frac_of_fp64_peak": useful_flops_step * args.steps * world / (ms * 1e-3) / 1e12 / (peak * world),
         "stage_ms_per_step": stage_ms,
-        "trajectory": {"gates": prep_gates, "ms": prep_ms, "gates_per_s": prep_gates / (prep_ms * 1e-3) if prep_ms > 0 else None},
-        "state": {"sum_n": total_n, "log_norm": ln, "discarded": stats["discarded"], "svd_sweeps_max": stats["sweeps"],
+        "trajectory": {"gates": res["prep_gates"], "ms": res["prep_ms"],
+                       "gates_per_s": res["prep_gates"] / (res["prep_ms"] * 1e-3) if res["prep_ms"] > 0 else None},
+        "state": {"sum_n": res["sum_n"], "log_norm": res["log_norm"], "discarded": stats["discarded"], "svd_sweeps_max": stats["sweeps"],
                   "svd_converged": stats["converged"]},
         "cpu_baseline": cpu,
+        "per_workload": per_workload,
     }
     print(json.dumps(out))
     if world > 1:
@@ -431,6 +530,7 @@ def main():
     ap.add_argument("--cpu-gates", type=int, default=96, help="oracle gates in the cpu_baseline sample")
     ap.add_argument("--ref-gates", type=int, default=8, help="oracle gates per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-workload", action="store_true", help="skip the shorter measurements of the other four configs")
     args = ap.parse_args()
     w = inputs.WORKLOADS[args.workload]
     if args.impl == "reference":

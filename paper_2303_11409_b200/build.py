@@ -12,6 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libu1mps.so")
 SOURCES = ["api.cu", "plan.cu", "contract.cu", "svd.cu", "select.cu", "readout.cu"]
+PROBE = os.path.join(HERE, "fp64_probe")          # measured FP64 peak (csrc/fp64_probe.cu), run by bench.py
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--extended-lambda",
          "-shared", "-Xcompiler", "-fPIC"]
 
@@ -35,6 +36,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed:\n" + res.stdout + res.stderr)
     if verbose:
         print(res.stderr)
+    res = subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", PROBE,
+                          os.path.join(CSRC, "fp64_probe.cu")], capture_output=True, text=True)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed (fp64_probe):\n" + res.stdout + res.stderr)
     return LIB
 
 

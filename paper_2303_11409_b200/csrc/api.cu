@@ -44,6 +44,7 @@ Sizes compute_sizes(int M, int d, int N, int chi) {
   add((size_t)M * chi * chi * 16);                               // gam
   add((size_t)M * NC * d * 8);                                   // gamoff
   add(8 * 8); add(8 * 4); add((M + 1) * 8); add(M * 4);          // scal, err, dout, occ
+  add((size_t)std::max(M, 1) * 8 * 8 + (size_t)U1_RD_SLICES * 8 + 4096); add((size_t)M * 4);   // a6 partial sums, slice counters
   add(z.Gmax * 4); add((size_t)z.Gmax * d * d * d * d * 16);     // site, U
   for (int i = 0; i < 5; ++i) add((E + 1) * 4);                  // rows cols keep blk tmpa
   add((E + 1) * 8); add((E + 1) * 4);                            // goff svoff
@@ -79,6 +80,7 @@ struct u1mps {
   Stage stage;
   int staged_site;
   double* dout;  // device scratch [M+1]
+  double* rd_part; size_t rd_cap; int* rd_count;   // a6: partial sums of the slices of a site, slices finished per site
   int* occ_dev;
   int last_site;
   cudaError_t cuda_err;
@@ -245,6 +247,8 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
   S.gamoff = A.take<long long>((size_t)M * NC * d);
   S.scal = A.take<double>(8); S.err = A.take<int>(8);
   h->dout = A.take<double>(M + 1); h->occ_dev = A.take<int>(M);
+  h->rd_cap = (size_t)std::max(M, 1) * 8 + U1_RD_SLICES + 512;
+  h->rd_part = A.take<double>(h->rd_cap); h->rd_count = A.take<int>(M);
   Plan& P = h->P;
   P.site = A.take<int>(z.Gmax); P.U = A.take<cplx>((size_t)z.Gmax * d * d * d * d);
   P.rows = A.take<int>(E + 1); P.cols = A.take<int>(E + 1); P.keep = A.take<int>(E + 1);
@@ -271,6 +275,7 @@ int u1mps_create(u1mps_t** out, int M, int d, int N, int chi, void* dev_arena, s
   if (e == cudaSuccess) e = cudaMemsetAsync(P.cnt, 0, 8 * 4, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(S.err, 0, 8 * 4, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(S.scal, 0, 8 * 8, h->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->rd_count, 0, (size_t)M * 4, h->stream);
   // empty bond tables and block offsets: a fresh handle may be filled by the import calls alone
   if (e == cudaSuccess) e = cudaMemsetAsync(S.nb, 0, (size_t)(M + 1) * NC * 4, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(S.ob, 0, (size_t)(M + 1) * NC * 4, h->stream);
@@ -410,7 +415,7 @@ int u1mps_expect_n_all(u1mps_t* h, double* out) {
   if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
-  u1_launch_expect_n(h->S, h->dout, h->L);
+  u1_launch_expect_n(h->S, 0, h->M, h->rd_part, h->rd_count, h->dout, h->L);
   CK(cudaGetLastError());
   CK(cudaMemcpyAsync(out, h->dout, (size_t)h->M * 8, cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
@@ -420,10 +425,11 @@ int u1mps_expect_n_all(u1mps_t* h, double* out) {
 int u1mps_expect_n(u1mps_t* h, int site, double* out) {
   if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out || site < 0 || site >= h->M) return U1MPS_EINVAL;
-  std::vector<double> all(h->M);
-  int r = u1mps_expect_n_all(h, all.data());
-  if (r) return r;
-  *out = all[site];
+  if (h->stage != ST_NONE) return U1MPS_ESTAGED;
+  u1_launch_expect_n(h->S, site, 1, h->rd_part, h->rd_count, h->dout, h->L);   // this site only, on all SMs
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, h->dout + site, 8, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
   return U1MPS_OK;
 }
 
@@ -431,7 +437,7 @@ int u1mps_bond_entropy_all(u1mps_t* h, double* out) {
   if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out) return U1MPS_EINVAL;
   if (h->stage != ST_NONE) return U1MPS_ESTAGED;
-  u1_launch_entropy(h->S, h->dout, h->L);
+  u1_launch_entropy(h->S, 0, h->M + 1, h->dout, h->L);
   CK(cudaGetLastError());
   CK(cudaMemcpyAsync(out, h->dout, (size_t)(h->M + 1) * 8, cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
@@ -441,10 +447,11 @@ int u1mps_bond_entropy_all(u1mps_t* h, double* out) {
 int u1mps_bond_entropy(u1mps_t* h, int bond, double* out) {
   if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out || bond < 0 || bond > h->M) return U1MPS_EINVAL;
-  std::vector<double> all(h->M + 1);
-  int r = u1mps_bond_entropy_all(h, all.data());
-  if (r) return r;
-  *out = all[bond];
+  if (h->stage != ST_NONE) return U1MPS_ESTAGED;
+  u1_launch_entropy(h->S, bond, 1, h->dout, h->L);
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, h->dout + bond, 8, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
   return U1MPS_OK;
 }
 

@@ -1,5 +1,6 @@
 // readout.cu — step a6 (canonical-form readouts, SURVEY §8(c) "Readouts"; Eq.10/15 canonical form)
 // and the small state-maintenance kernels (product state, block-offset rebuild after an import).
+#include <algorithm>
 #include "common.cuh"
 
 #define RD_THREADS 256
@@ -17,40 +18,85 @@ __device__ __forceinline__ double block_sum(double v, double* sh) {
   return r;
 }
 
-// <n_s> = sum_{cl,cr} (cl - cr) sum_{a,b} lamL[cl]_a^2 |Gamma[cl,cr]_ab|^2 lamR[cr]_b^2 ; one CTA per site
-__global__ void __launch_bounds__(RD_THREADS) expect_n_kernel(DevState S, double* out) {
-  __shared__ double sh[RD_THREADS];
-  const int s = blockIdx.x, NC = S.NC, d = S.d;
+// <n_s> = sum_{cl,cr} (cl - cr) sum_{a,b} lamL[cl]_a^2 |Gamma[cl,cr]_ab|^2 lamR[cr]_b^2   (canonical form, Eq.10/15)
+// Memory-bound: every Gamma block with occupation >= 1 is read once.  The rows of all such blocks of a site form one
+// virtual row space; slice j of K of it belongs to CTA (site, j) - K is chosen by the host so that all SMs are busy
+// whatever M is - one warp per row, lanes along the row (coalesced 16-byte loads), shuffle reductions.  The K partial
+// sums of a site are added in slice order by the last CTA of the site: the result does not depend on timing.
+#define RD_MAXBLK 1024   // (cl, i) blocks of a site held in shared memory at a time (more are processed in batches)
+__global__ void __launch_bounds__(RD_THREADS) expect_n_kernel(DevState S, int site0, int K, double* part, int* count, double* out) {
+  __shared__ int s_pref[RD_MAXBLK + 1];        // virtual row prefix over the blocks of the batch
+  __shared__ int s_cl[RD_MAXBLK];               // block -> cl * d + i
+  __shared__ double s_red[RD_THREADS / 32];
+  __shared__ int s_nblk, s_last;
+  const int s = site0 + blockIdx.x / K, j = blockIdx.x % K, NC = S.NC, d = S.d;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int* nbL = S.nb + (long long)s * NC;
   const int* nbR = S.nb + (long long)(s + 1) * NC;
-  double acc = 0.0;
-  for (int cl = 0; cl < NC; ++cl) {
-    const int nl = nbL[cl];
-    if (nl == 0) continue;
-    const double* lamL = S.lam + (long long)s * S.chi + S.ob[(long long)s * NC + cl];
-    for (int i = 1; i < d && cl - i >= 0; ++i) {  // occupation i = 0 contributes nothing
-      const int cr = cl - i, nr = nbR[cr];
-      if (nr == 0) continue;
-      const double* lamR = S.lam + (long long)(s + 1) * S.chi + S.ob[(long long)(s + 1) * NC + cr];
-      const cplx* Gm = S.gam + (long long)s * S.gcap + S.gamoff[((long long)s * NC + cl) * d + i];
-      double part = 0.0;
-      for (long long idx = threadIdx.x; idx < (long long)nl * nr; idx += RD_THREADS) {
-        const int a = (int)(idx / nr), b = (int)(idx % nr);
-        const cplx v = Gm[idx];
-        const double la = lamL[a], lb = lamR[b];
-        part = fma((v.x * v.x + v.y * v.y) * (la * la), lb * lb, part);
+  const cplx* gam = S.gam + (long long)s * S.gcap;
+  const long long* goff = S.gamoff + (long long)s * NC * d;
+  const double* lamL0 = S.lam + (long long)s * S.chi;
+  const double* lamR0 = S.lam + (long long)(s + 1) * S.chi;
+  const int* obL = S.ob + (long long)s * NC;
+  const int* obR = S.ob + (long long)(s + 1) * NC;
+  double acc = 0.0;   // this warp's sum
+  for (int f0 = 0; f0 < NC * d; f0 += RD_MAXBLK) {   // batches of candidate (cl, i) pairs (one batch unless NC * d > 1024)
+    __syncthreads();
+    if (tid == 0) {
+      int nb = 0, run = 0;
+      for (int f = f0; f < min(NC * d, f0 + RD_MAXBLK); ++f) {
+        const int cl = f / d, i = f - cl * d;
+        if (i == 0 || cl - i < 0 || nbL[cl] == 0 || nbR[cl - i] == 0) continue;   // occupation 0 contributes nothing
+        s_pref[nb] = run; s_cl[nb] = f; run += nbL[cl]; ++nb;
       }
-      acc = fma((double)i, part, acc);
+      s_pref[nb] = run; s_nblk = nb;
+    }
+    __syncthreads();
+    const int nblk = s_nblk, rtot = s_pref[nblk];
+    // rows [r0, r1) of the virtual row space belong to this slice; warps take them round-robin
+    const int r0 = (int)((long long)rtot * j / K), r1 = (int)((long long)rtot * (j + 1) / K);
+    int bi = 0;
+    for (int r = r0 + warp; r < r1; r += RD_THREADS / 32) {
+      while (s_pref[bi + 1] <= r) ++bi;          // rows ascend: linear advance
+      const int f = s_cl[bi], cl = f / d, i = f - cl * d, cr = cl - i;
+      const int a = r - s_pref[bi], nr = nbR[cr];
+      const cplx* row = gam + goff[f] + (long long)a * nr;
+      const double* lamR = lamR0 + obR[cr];
+      double p = 0.0;
+      for (int b = lane; b < nr; b += 32) {
+        const cplx v = __ldcs(row + b);
+        const double lb = lamR[b];
+        p = fma(fma(v.x, v.x, v.y * v.y), lb * lb, p);
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) p += __shfl_xor_sync(0xffffffffu, p, o);
+      const double la = lamL0[obL[cl] + a];
+      acc = fma((double)i * (la * la), p, acc);
     }
   }
-  const double tot = block_sum(acc, sh);
-  if (threadIdx.x == 0) out[s] = tot;
+  if (lane == 0) s_red[warp] = acc;
+  __syncthreads();
+  if (tid == 0) {
+    double t = 0.0;
+    for (int w = 0; w < RD_THREADS / 32; ++w) t += s_red[w];
+    part[(long long)(s - site0) * K + j] = t;
+    __threadfence();
+    s_last = (atomicAdd(&count[s - site0], 1) == K - 1) ? 1 : 0;
+  }
+  __syncthreads();
+  if (s_last && tid == 0) {   // the slices of the site, in slice order
+    __threadfence();
+    double t = 0.0;
+    for (int jj = 0; jj < K; ++jj) t += __ldcg(&part[(long long)(s - site0) * K + jj]);
+    out[s] = t;
+    count[s - site0] = 0;     // ready for the next launch
+  }
 }
 
 // S_k = - sum lambda^2 ln lambda^2 ; one CTA per bond
-__global__ void __launch_bounds__(RD_THREADS) entropy_kernel(DevState S, double* out) {
+__global__ void __launch_bounds__(RD_THREADS) entropy_kernel(DevState S, int bond0, double* out) {
   __shared__ double sh[RD_THREADS];
-  const int k = blockIdx.x, NC = S.NC;
+  const int k = bond0 + blockIdx.x, NC = S.NC;
   int D = 0;
   for (int c = 0; c < NC; ++c) D += S.nb[(long long)k * NC + c];
   double acc = 0.0;
@@ -107,15 +153,17 @@ __global__ void product_state_kernel(DevState S, const int* occ) {
   }
 }
 
-void u1_launch_expect_n(const DevState& S, double* out_dev, const LaunchCfg& L) {
+void u1_launch_expect_n(const DevState& S, int site0, int nsites, double* part, int* count, double* out_dev, const LaunchCfg& L) {
+  // K slices per site so that about 8 CTAs per SM exist whatever the number of sites is
+  const int K = std::max(1, std::min(U1_RD_SLICES, (8 * L.sms + nsites - 1) / nsites));
   L.prof->begin(U1_ST_READOUT, L.stream);
-  expect_n_kernel<<<S.M, RD_THREADS, 0, L.stream>>>(S, out_dev);
+  expect_n_kernel<<<nsites * K, RD_THREADS, 0, L.stream>>>(S, site0, K, part, count, out_dev);
   L.prof->end(L.stream);
   ++*L.launches;
 }
-void u1_launch_entropy(const DevState& S, double* out_dev, const LaunchCfg& L) {
+void u1_launch_entropy(const DevState& S, int bond0, int nbonds, double* out_dev, const LaunchCfg& L) {
   L.prof->begin(U1_ST_READOUT, L.stream);
-  entropy_kernel<<<S.M + 1, RD_THREADS, 0, L.stream>>>(S, out_dev);
+  entropy_kernel<<<nbonds, RD_THREADS, 0, L.stream>>>(S, bond0, out_dev);
   L.prof->end(L.stream);
   ++*L.launches;
 }
