@@ -23,6 +23,7 @@ __device__ __forceinline__ double block_sum(double v, double* sh) {
 // virtual row space; slice j of K of it belongs to CTA (site, j) - K is chosen by the host so that all SMs are busy
 // whatever M is - one warp per row, lanes along the row (coalesced 16-byte loads), shuffle reductions.  The K partial
 // sums of a site are added in slice order by the last CTA of the site: the result does not depend on timing.
+#define RD_UNR 8          // 16-byte loads in flight per thread
 #define RD_MAXBLK 1024   // (cl, i) blocks of a site held in shared memory at a time (more are processed in batches)
 __global__ void __launch_bounds__(RD_THREADS) expect_n_kernel(DevState S, int site0, int K, double* part, int* count, double* out) {
   __shared__ int s_pref[RD_MAXBLK + 1];        // virtual row prefix over the blocks of the batch
@@ -39,41 +40,64 @@ __global__ void __launch_bounds__(RD_THREADS) expect_n_kernel(DevState S, int si
   const double* lamR0 = S.lam + (long long)(s + 1) * S.chi;
   const int* obL = S.ob + (long long)s * NC;
   const int* obR = S.ob + (long long)(s + 1) * NC;
-  double acc = 0.0;   // this warp's sum
+  double acc = 0.0;   // this thread's sum
   for (int f0 = 0; f0 < NC * d; f0 += RD_MAXBLK) {   // batches of candidate (cl, i) pairs (one batch unless NC * d > 1024)
+    __syncthreads();
+    // rows of every candidate block (0: absent, or occupation 0, which contributes nothing), all threads; then one
+    // thread compacts the list out of shared memory
+    for (int f = f0 + tid; f < min(NC * d, f0 + RD_MAXBLK); f += RD_THREADS) {
+      const int cl = f / d, i = f - cl * d;
+      s_cl[f - f0] = (i == 0 || cl - i < 0 || nbR[cl - i] == 0) ? 0 : nbL[cl];
+    }
     __syncthreads();
     if (tid == 0) {
       int nb = 0, run = 0;
       for (int f = f0; f < min(NC * d, f0 + RD_MAXBLK); ++f) {
-        const int cl = f / d, i = f - cl * d;
-        if (i == 0 || cl - i < 0 || nbL[cl] == 0 || nbR[cl - i] == 0) continue;   // occupation 0 contributes nothing
-        s_pref[nb] = run; s_cl[nb] = f; run += nbL[cl]; ++nb;
+        const int rows = s_cl[f - f0];
+        if (rows == 0) continue;
+        s_pref[nb] = run; s_cl[nb] = f; run += rows; ++nb;   // nb <= f - f0: the compacted list never overtakes the scan
       }
       s_pref[nb] = run; s_nblk = nb;
     }
     __syncthreads();
     const int nblk = s_nblk, rtot = s_pref[nblk];
-    // rows [r0, r1) of the virtual row space belong to this slice; warps take them round-robin
+    // rows [r0, r1) of the virtual row space belong to this slice.  Inside a block these rows are one contiguous array:
+    // the CTA streams it flat (thread t takes elements t, t + 256, ...: fully coalesced whatever the row length is),
+    // row and column of an element from its index by a single-precision reciprocal (exact below 2^24) with a +-1 fix-up
     const int r0 = (int)((long long)rtot * j / K), r1 = (int)((long long)rtot * (j + 1) / K);
     int bi = 0;
-    for (int r = r0 + warp; r < r1; r += RD_THREADS / 32) {
-      while (s_pref[bi + 1] <= r) ++bi;          // rows ascend: linear advance
+    while (bi < nblk && s_pref[bi + 1] <= r0) ++bi;
+    for (; bi < nblk && s_pref[bi] < r1; ++bi) {
       const int f = s_cl[bi], cl = f / d, i = f - cl * d, cr = cl - i;
-      const int a = r - s_pref[bi], nr = nbR[cr];
-      const cplx* row = gam + goff[f] + (long long)a * nr;
+      const int ra = max(r0, s_pref[bi]) - s_pref[bi], rb = min(r1, s_pref[bi + 1]) - s_pref[bi];
+      const int nr = nbR[cr];
+      const cplx* blk = gam + goff[f] + (long long)ra * nr;
+      const double* lamL = lamL0 + obL[cl] + ra;
       const double* lamR = lamR0 + obR[cr];
+      const int ne = (rb - ra) * nr;              // <= chi^2 = 2^24
+      const float inv = 1.0f / (float)nr;
       double p = 0.0;
-      for (int b = lane; b < nr; b += 32) {
-        const cplx v = __ldcs(row + b);
-        const double lb = lamR[b];
-        p = fma(fma(v.x, v.x, v.y * v.y), lb * lb, p);
-      }
+      for (int e0 = tid; e0 < ne; e0 += RD_UNR * RD_THREADS) {
+        cplx v[RD_UNR]; double w[RD_UNR];
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) p += __shfl_xor_sync(0xffffffffu, p, o);
-      const double la = lamL0[obL[cl] + a];
-      acc = fma((double)i * (la * la), p, acc);
+        for (int x = 0; x < RD_UNR; ++x) {
+          const int idx = e0 + x * RD_THREADS;
+          const bool ok = idx < ne;
+          v[x] = ok ? __ldcs(blk + idx) : make_double2(0.0, 0.0);
+          int ar = __float2int_rz((float)idx * inv), br = idx - ar * nr;
+          if (br >= nr) { br -= nr; ++ar; } else if (br < 0) { br += nr; --ar; }
+          const double la = ok ? lamL[ar] : 0.0, lb = ok ? lamR[br] : 0.0;
+          w[x] = (la * la) * (lb * lb);
+        }
+#pragma unroll
+        for (int x = 0; x < RD_UNR; ++x) p = fma(fma(v[x].x, v[x].x, v[x].y * v[x].y), w[x], p);
+      }
+      acc = fma((double)i, p, acc);
     }
   }
+  // deterministic sum over the CTA: lanes by shuffle, warps in order
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
   if (lane == 0) s_red[warp] = acc;
   __syncthreads();
   if (tid == 0) {
@@ -154,8 +178,10 @@ __global__ void product_state_kernel(DevState S, const int* occ) {
 }
 
 void u1_launch_expect_n(const DevState& S, int site0, int nsites, double* part, int* count, double* out_dev, const LaunchCfg& L) {
-  // K slices per site so that about 8 CTAs per SM exist whatever the number of sites is
-  const int K = std::max(1, std::min(U1_RD_SLICES, (8 * L.sms + nsites - 1) / nsites));
+  // K slices per site so that the grid is one full wave of resident CTAs whatever the number of sites is
+  static int occ = 0;
+  if (occ == 0 && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, expect_n_kernel, RD_THREADS, 0) != cudaSuccess) occ = 4;
+  const int K = std::max(1, std::min(U1_RD_SLICES, (std::max(occ, 1) * L.sms) / nsites));
   L.prof->begin(U1_ST_READOUT, L.stream);
   expect_n_kernel<<<nsites * K, RD_THREADS, 0, L.stream>>>(S, site0, K, part, count, out_dev);
   L.prof->end(L.stream);

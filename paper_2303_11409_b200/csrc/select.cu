@@ -124,71 +124,55 @@ __global__ void __launch_bounds__(SEL_THREADS) select_kernel(DevState S, Plan P,
   }
 }
 
-// a5 tile list over (entry, part) restricted to the KEPT singular vectors (the planner sized it for all min(rows, cols)
-// of them before a4 had decided): V(c) rows x keep, W(c) keep x cols.  One CTA, exclusive scan into P.t5pref.
+// a5 work list over (entry, part) restricted to sectors that KEEP singular vectors (the planner sized it before a4 had
+// decided): strips of U1_TILE bond indices - rows of V(c), columns of W(c) - each strip runs over all kept vectors.
+// One CTA, exclusive scan into P.t5pref.
 __global__ void __launch_bounds__(SEL_THREADS) retile_kernel(Plan P, int L /* = 2 G NC */) {
   __shared__ int sh[SEL_THREADS];
   auto tiles = [&](int f) {
     const int e = f >> 1, k = P.keep[e];
     if (k == 0) return 0;
-    return (f & 1) ? u1_ceil_div(k, U1_TILE) * u1_ceil_div(P.cols[e], U1_TILE) : u1_ceil_div(P.rows[e], U1_TILE) * u1_ceil_div(k, U1_TILE);
+    return (f & 1) ? u1_ceil_div(P.cols[e], U1_TILE) : u1_ceil_div(P.rows[e], U1_TILE);
   };
   u1_block_excl_scan<int, SEL_THREADS>(tiles, P.t5pref, L, sh);
   if (threadIdx.x == 0) P.cnt[5] = P.t5pref[L];
 }
 
 #define SC_THREADS 256
-#define SC_RUN 16
-// a5: 32 x 32 tiles of V(c) (part 0) and W(c) (part 1) out of the stacked Jacobi matrices into the block-sparse Gammas.
-// Per tile, 64 threads first work out what is constant along a tile row / column (source column and 1/sigma of the 32
-// singular vectors; destination block, offset and 1/lambda of the 32 bond indices) into shared memory, so that the
-// two bulk passes are load - multiply - store only: coalesced 512-byte column segments in, 512-byte row segments out.
+#define SC_VW 64   // singular vectors per pass of a strip
+// a5: V(c) (part 0) and W(c) (part 1) out of the stacked Jacobi matrices into the block-sparse Gammas, in strips of 32
+// bond indices (rows a of V, columns b of W) x all kept singular vectors.  What is constant along a bond index -
+// destination block, offset and 1/lambda (Eq.13/14) - is worked out once per strip by 32 threads; per pass of 64
+// vectors another 64 threads fetch the source column and 1/sigma of each; the bulk is then load - multiply - store:
+// coalesced 512-byte column segments in, 512- / 1024-byte row segments out (V is transposed through shared memory).
 __global__ void __launch_bounds__(SC_THREADS) scatter_kernel(DevState S, Plan P, int G) {
-  __shared__ cplx tile[U1_TILE][U1_TILE + 1];
-  __shared__ long long s_src[U1_TILE];   // per singular vector jj: offset of its column in the stacked matrix (-1: not kept)
-  __shared__ double s_isg[U1_TILE];      // ... 1/sigma (or 1 where the vectors are the unit-norm J columns)
+  __shared__ cplx tile[SC_VW][U1_TILE + 1];
+  __shared__ long long s_src[SC_VW];     // per singular vector jj: offset of its column in the stacked matrix (-1: not kept)
+  __shared__ double s_isg[SC_VW];        // ... 1/sigma (or 1 where the vectors are the unit-norm J columns)
   __shared__ long long s_dst[U1_TILE];   // per bond index (row a of V / column b of W): destination offset (-1: outside)
   __shared__ double s_ilm[U1_TILE];      // ... 1/lambda of that bond index (Eq.13/14)
   __shared__ int s_ldd[U1_TILE];         // ... row length of the destination block (part 1)
   const int NC = S.NC, d = S.d;
   const int nf = G * NC * 2, total = P.cnt[5];
   const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
-  // tiles are handed out in runs of SC_RUN consecutive tiles: one binary search of the tile prefix per run (13 dependent
-  // L2 loads), then a linear advance
-  for (int run = blockIdx.x; run * SC_RUN < total; run += gridDim.x) {
-   int f = 0;
-   {
-    int lo = 0, hi = nf;
-    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (P.t5pref[mid] <= run * SC_RUN) lo = mid; else hi = mid; }
-    f = lo;
-   }
-   for (int t = run * SC_RUN; t < min(total, (run + 1) * SC_RUN); ++t) {
-    while (P.t5pref[f + 1] <= t) ++f;
+  for (int unit = blockIdx.x; unit < total; unit += gridDim.x) {
+    int f;
+    {
+      int lo = 0, hi = nf;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (P.t5pref[mid] <= unit) lo = mid; else hi = mid; }
+      f = lo;
+    }
     const int e = f >> 1, part = f & 1;
     const int g = e / NC, c = e % NC, s = P.site[g];
     const int rows = P.rows[e], cols = P.cols[e], m = max(rows, cols), n = min(rows, cols), ld = m + n;
     const bool tr = rows < cols;
     const int keep = P.keep[e];
-    const int local = t - P.t5pref[f];
     const cplx* W = P.W + P.goff[e];
     const int so = P.svoff[e];
-    const int tcols = u1_ceil_div(part == 0 ? keep : cols, U1_TILE);
-    // part 0: tile rows = bond indices a of the left bond, tile columns = singular vectors; part 1: the other way round
-    const int x0 = (local / tcols) * U1_TILE, y0 = (local % tcols) * U1_TILE;
-    const int j0 = part == 0 ? y0 : x0, i0 = part == 0 ? x0 : y0;
-    if (j0 >= keep) continue;  // (block-uniform)
-    __syncthreads();
-    if (tid < U1_TILE) {  // singular vector j0 + tid
-      const int pj = j0 + tid;
-      long long src = -1; double isg = 1.0;
-      if (pj < keep) {
-        src = (long long)P.perm[so + pj] * ld;
-        // V = G / sigma when G holds Theta (rows >= cols), W = conj(G) / sigma when it holds Theta^H
-        if ((part == 0) != tr) isg = 1.0 / P.svs[so + pj];
-      }
-      s_src[tid] = src; s_isg[tid] = isg;
-    } else if (tid < 2 * U1_TILE) {  // bond index i0 + (tid - 32): row a of V (left bond) or column b of W (right bond)
-      const int k = tid - U1_TILE, idx = i0 + k;
+    const int i0 = (unit - P.t5pref[f]) * U1_TILE;   // first bond index of the strip
+    __syncthreads();   // the previous strip is done with the shared arrays
+    if (tid < U1_TILE) {  // bond index i0 + tid: row a of V (left bond) or column b of W (right bond)
+      const int idx = i0 + tid;
       long long dst = -1; double ilm = 0.0; int ldd = 0;
       if (part == 0 && idx < rows) {
         const int* nbL = S.nb + (long long)s * NC;
@@ -208,48 +192,72 @@ __global__ void __launch_bounds__(SC_THREADS) scatter_kernel(DevState S, Plan P,
         dst = (long long)(s + 1) * S.gcap + S.gamoff[((long long)(s + 1) * NC + c) * d + (c - cr)] + bl;
         ldd = nbR[cr];
       }
-      s_dst[k] = dst; s_ilm[k] = ilm; s_ldd[k] = ldd;
+      s_dst[tid] = dst; s_ilm[tid] = ilm; s_ldd[tid] = ldd;
     }
-    __syncthreads();
-    if (part == 0) {
-      // V(c)[a, jj] = G[a, p] / sigma (rows >= cols) or J[a, p]: read 32 rows of 32 columns, transpose, write rows
-      const int roff = tr ? m : 0;
-      for (int jj = ty; jj < U1_TILE; jj += SC_THREADS / 32) {
-        cplx v = make_double2(0.0, 0.0);
-        const long long src = s_src[jj];
-        if (src >= 0 && i0 + tx < rows) {
-          v = __ldcg(W + src + roff + i0 + tx);
-          const double sc = s_isg[jj];
-          v.x *= sc; v.y *= sc;
+    for (int j0 = 0; j0 < keep; j0 += SC_VW) {
+      __syncthreads();   // the previous pass is done with tile / s_src (and the strip's arrays are in place)
+      if (tid >= SC_THREADS - SC_VW) {  // singular vector j0 + k
+        const int k = tid - (SC_THREADS - SC_VW), pj = j0 + k;
+        long long src = -1; double isg = 1.0;
+        if (pj < keep) {
+          src = (long long)P.perm[so + pj] * ld;
+          // V = G / sigma when G holds Theta (rows >= cols), W = conj(G) / sigma when it holds Theta^H
+          if ((part == 0) != tr) isg = 1.0 / P.svs[so + pj];
         }
-        tile[jj][tx] = v;
+        s_src[k] = src; s_isg[k] = isg;
       }
       __syncthreads();
-      for (int aa = ty; aa < U1_TILE; aa += SC_THREADS / 32) {
-        const long long dst = s_dst[aa];
-        if (dst >= 0 && j0 + tx < keep) {
-          cplx v = tile[tx][aa];
-          const double il = s_ilm[aa];
-          v.x *= il; v.y *= il;
-          S.gam[dst + j0 + tx] = v;
+      if (part == 0) {
+        // V(c)[a, jj] = G[a, p] / sigma (rows >= cols) or J[a, p]: read 32 rows of 64 columns, transpose, write rows
+        const int roff = tr ? m : 0;
+        cplx v[SC_VW / (SC_THREADS / 32)];   // all loads of the pass in flight before the first use
+#pragma unroll
+        for (int x = 0; x < SC_VW / (SC_THREADS / 32); ++x) {
+          const long long src = s_src[ty + x * (SC_THREADS / 32)];
+          v[x] = (src >= 0 && i0 + tx < rows) ? __ldcs(W + src + roff + i0 + tx) : make_double2(0.0, 0.0);
         }
-      }
-    } else {
-      // W(c)[jj, b] = conj(J[b, p]) (rows >= cols) or conj(G[b, p]) / sigma: no transposition needed
-      const int roff = tr ? 0 : m;
-      const long long dst = s_dst[tx];
-      const double il = s_ilm[tx];
-      const int ldd = s_ldd[tx];
-      for (int jj = ty; jj < U1_TILE; jj += SC_THREADS / 32) {
-        const long long src = s_src[jj];
-        if (src >= 0 && dst >= 0) {
-          cplx v = __ldcg(W + src + roff + i0 + tx);
-          const double sc = s_isg[jj] * il;
-          S.gam[dst + (long long)(j0 + jj) * ldd] = make_double2(v.x * sc, -v.y * sc);
+#pragma unroll
+        for (int x = 0; x < SC_VW / (SC_THREADS / 32); ++x) {
+          const int jj = ty + x * (SC_THREADS / 32);
+          const double sc = s_isg[jj];
+          tile[jj][tx] = make_double2(v[x].x * sc, v[x].y * sc);
+        }
+        __syncthreads();
+        for (int aa = ty; aa < U1_TILE; aa += SC_THREADS / 32) {
+          const long long dst = s_dst[aa];
+          const double il = s_ilm[aa];
+#pragma unroll
+          for (int h = 0; h < SC_VW / 32; ++h) {
+            const int jj = tx + 32 * h;
+            if (dst >= 0 && j0 + jj < keep) {
+              cplx v = tile[jj][aa];
+              v.x *= il; v.y *= il;
+              __stcs(&S.gam[dst + j0 + jj], v);
+            }
+          }
+        }
+      } else {
+        // W(c)[jj, b] = conj(J[b, p]) (rows >= cols) or conj(G[b, p]) / sigma: no transposition needed
+        const int roff = tr ? 0 : m;
+        const long long dst = s_dst[tx];
+        const double il = s_ilm[tx];
+        const int ldd = s_ldd[tx];
+        cplx v[SC_VW / (SC_THREADS / 32)];
+#pragma unroll
+        for (int x = 0; x < SC_VW / (SC_THREADS / 32); ++x) {
+          const long long src = s_src[ty + x * (SC_THREADS / 32)];
+          v[x] = (src >= 0 && dst >= 0) ? __ldcs(W + src + roff + i0 + tx) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int x = 0; x < SC_VW / (SC_THREADS / 32); ++x) {
+          const int jj = ty + x * (SC_THREADS / 32);
+          if (s_src[jj] >= 0 && dst >= 0) {
+            const double sc = s_isg[jj] * il;
+            __stcs(&S.gam[dst + (long long)(j0 + jj) * ldd], make_double2(v[x].x * sc, -v[x].y * sc));
+          }
         }
       }
     }
-   }
   }
 }
 
