@@ -264,7 +264,7 @@ __device__ __forceinline__ uchar2 mod_pivot(int rho, int k, int n) {
   return make_uchar2((unsigned char)p, (unsigned char)q);
 }
 
-__device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2* tab, int hp, double tol2, int* inner, int inner_max, int g, int gtid) {
+__device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2* tab, int hp, double tol2, int* inner, int inner_max, double quad, int g, int gtid) {
   const int tid = gtid;
   const int np2 = 2 * hp;
   for (int idx = tid; idx < np2 * hp; idx += SV_GROUP) tab[idx] = mod_pivot(idx / hp, idx % hp, np2);
@@ -415,7 +415,7 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
     }
     if (!sweep_any) break;
     ++*inner;
-    if (!gsync_or(g, mymax > SV_QUAD)) break;
+    if (!gsync_or(g, mymax > quad)) break;
   }
   if (pend && tid >= 32) q_update(Rm + (cur ^ 1) * U1_PB, prow);
   gsync(g);
@@ -480,6 +480,68 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
   }
   cp_async_wait<0>();
   gsync(g);
+}
+
+// A sector of at most two panels (n <= 32) is a single item - all its columns - and depends on nothing: in a launch
+// that consists of such sectors only (tiny bonds: the first layers of every trajectory, BASELINE.json's config 1) the CTA
+// that draws a sector's ticket of round 0 iterates it to convergence on the spot: Gram - EVD run to convergence -
+// update, until a visit finds nothing to rotate or only rotations in the quadratic regime.  Returns the visits made,
+// negative if the limit was hit.  (A kernel of its own, svd_solo_kernel, launched in front of svd_kernel: it returns at
+// once unless the launch consists of such sectors only, and svd_kernel then finds every sector finished.)
+__device__ __forceinline__ int solo_sector(const Plan& P, int e, cplx* stages, cplx* Hs, cplx* Qs, double4* Rm, uchar2* tab, int* s_col,
+                                        int inner_max, int R) {
+  const int gtid = threadIdx.x, g = 0;
+  Item I;
+  const int r = P.rows[e], q = P.cols[e], n = min(r, q);
+  I.m = max(r, q);
+  I.mt = I.m + n;
+  I.W = P.W + P.goff[e];
+  I.ca = 0; I.na = min(U1_PB, n);
+  I.cb = U1_PB; I.nb = max(0, min(U1_PB, n - U1_PB));
+  const double tol = SV_TOLFAC * 1.1102230246251565e-16 * sqrt((double)I.m);
+  I.tol2 = tol * tol;
+  if (gtid < SV_W) {
+    const int j = gtid;
+    const bool ok = j < U1_PB ? j < I.na : j - U1_PB < I.nb;
+    s_col[j] = ok ? P.perm[P.svoff[e] + j] : 0;
+  }
+  I.col = s_col;
+  gsync(g);
+  const Loader L = make_loader(I, gtid);
+  for (int iter = 0; iter < U1_MAXSWEEP; ++iter) {
+    gram_phase(stages, Hs, I, L, g, gtid);
+    int todo = 0, big = 0;
+    for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
+      const int p = idx >> 5, qq = idx & 31;
+      if (p < qq) {
+        const double a = Hs[p * SV_HLD + p].x, b = Hs[qq * SV_HLD + qq].x;
+        const cplx gg = Hs[p * SV_HLD + qq];
+        const double ab = a * b, g2 = gg.x * gg.x + gg.y * gg.y;
+        if (ab > 0.0 && g2 > 1e-290) {
+          todo |= (g2 > I.tol2 * ab) ? 1 : 0;
+          big |= (g2 > SV_LASTPASS * ab) ? 1 : 0;
+        }
+      }
+    }
+    todo = gsync_or(g, todo);
+    big = gsync_or(g, big);
+    __syncthreads();
+    if (!todo) return iter + 1;
+    int inner = 0;
+    evd_phase(Hs, Qs, Rm, tab, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max + 4, 0.0, g, gtid);
+    __syncthreads();
+    update_phase(stages, Qs, I, L, g, gtid);
+    __syncthreads();   // the update's stores are visible to the CTA's next Gram pass
+    if (gtid == 0) {
+      const int sw = min(iter, U1_MAXSWEEP - 1);
+      long long t1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+      atomicMax(&P.trace[1 + sw], t1);
+      atomicAdd((unsigned long long*)&P.trace[1 + U1_MAXSWEEP + sw], 1ull);
+      atomicAdd((unsigned long long*)&P.trace[1 + 2 * U1_MAXSWEEP + sw], (unsigned long long)inner);
+    }
+    if (!big) return iter + 1;
+  }
+  return -1;
 }
 
 __device__ __forceinline__ int ld_acquire(const int* p) {
@@ -635,7 +697,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
       __syncthreads();
       SV_TICK(0);
       int inner = 0;
-      if (todo) evd_phase(Hs, Qs, Rm, tab, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, g, gtid);
+      if (todo) evd_phase(Hs, Qs, Rm, tab, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, SV_QUAD, g, gtid);
       __syncthreads();
       SV_TICK(2);
       if (todo) update_phase(stages, Qs, I, L, g, gtid);
@@ -694,6 +756,32 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
   }
 }
 
+__global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_solo_kernel(Plan P, int G, int NC, int inner_max) {
+  extern __shared__ __align__(16) unsigned char smraw[];
+  __shared__ int s_col[SV_W];
+  const int nblk = P.cnt[0], maxP = P.cnt[3];
+  if (maxP > 2 || nblk == 0) return;
+  cplx* stages = reinterpret_cast<cplx*>(smraw);
+  cplx* Hs = stages;
+  cplx* Qs = Hs + SV_W * SV_HLD;
+  double4* Rm = reinterpret_cast<double4*>(Qs + SV_W * SV_QLD);
+  uchar2* tab = reinterpret_cast<uchar2*>(Rm + 2 * U1_PB);
+  const int R = max(maxP, 1), E = G * NC;
+  int* done_at = P.flags + E;
+  for (int bi = blockIdx.x; bi < nblk; bi += gridDim.x) {
+    const int e = P.blk[bi];
+    __syncthreads();
+    const int visits = solo_sector(P, e, stages, Hs, Qs, Rm, tab, s_col, inner_max, R);
+    __syncthreads();
+    if (threadIdx.x == 0 && visits > 0) {   // (a sector that hit the limit stays unfinished: svd_kernel reports it)
+      atomicMin(&done_at[e], visits * R - 1);
+      atomicMax(&P.sched[4], visits * R - 1);
+      __threadfence();
+      atomicAdd(&P.sched[2], 1);
+    }
+  }
+}
+
 // sigma_j = norm of column j of G (top m rows), then sort each sector descending (ties: lower
 // column first).  One CTA per sector; bitonic sort in shared memory (n <= 4096).
 #define SORT_THREADS 1024
@@ -741,6 +829,8 @@ cudaError_t u1_svd_configure(int* grid, int* smem_bytes, int sms) {
   const int smem = SV_SMEM_BYTES;
   cudaError_t err = cudaFuncSetAttribute(svd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (err != cudaSuccess) return err;
+  err = cudaFuncSetAttribute(svd_solo_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (err != cudaSuccess) return err;
   err = cudaFuncSetAttribute(sigma_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, U1MPS_SORT_MAX * 12);
   if (err != cudaSuccess) return err;
   int occ = 0;
@@ -766,6 +856,7 @@ cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchC
   if (getenv("SV_PROFILE_CTAS")) grid = L.sms * atoi(getenv("SV_PROFILE_CTAS"));
 #endif
   L.prof->begin(U1_ST_SVD, L.stream);
+  svd_solo_kernel<<<L.sms * 2, U1_SVD_THREADS, (size_t)L.svd_smem, L.stream>>>(P, G, S.NC, inner_max);
   cudaError_t err = cudaLaunchCooperativeKernel((void*)svd_kernel, dim3(grid), dim3(U1_SVD_THREADS), args,
                                                 (size_t)L.svd_smem, L.stream);
   L.prof->end(L.stream);
@@ -773,6 +864,6 @@ cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchC
   L.prof->begin(U1_ST_SORT, L.stream);
   sigma_sort_kernel<<<L.sms * 2, SORT_THREADS, U1MPS_SORT_MAX * 12, L.stream>>>(P);
   L.prof->end(L.stream);
-  *L.launches += 3;
+  *L.launches += 4;
   return cudaGetLastError();
 }
