@@ -351,9 +351,16 @@ def measure(w, args, steps, warmup, prep_columns, with_e2e, rank, world, local, 
         a6 = {"ms_per_step": a6_ms / steps, "launches_per_step": a6_n / steps, "bytes_per_step": readout_bytes(gpu, w)}
     gpu.profile_enable(False)
     stats = gpu.last_stats()
+    full = None
+    if with_e2e:   # full-environment read-out (exact after truncation): sum_k <n_k> = N is the check, timed once
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        n_full = gpu.expect_n_full()
+        full = {"sum_n_full": float(np.sum(n_full)), "max_abs_diff_to_canonical": float(np.max(np.abs(n_full - n_k))),
+                "seconds": time.perf_counter() - t0}
     res = {"w": w, "ms": ms, "ms_e2e": ms_e2e, "launches": launches, "prof": prof, "clocks": clocks, "work": work,
            "work_after": work_after, "gates_per_step": gates_per_step, "prep_ms": prep_ms, "prep_gates": prep_gates,
-           "n_prep": n_prep, "stats": stats, "sum_n": float(np.sum(n_k)), "log_norm": ln, "a6": a6, "steps": steps}
+           "n_prep": n_prep, "stats": stats, "sum_n": float(np.sum(n_k)), "log_norm": ln, "a6": a6, "steps": steps, "full": full}
     gpu.close()
     del gpu, dev_cols, pin_cols
     torch.cuda.empty_cache()
@@ -510,7 +517,7 @@ def run_ours(args, w):
         "trajectory": {"gates": res["prep_gates"], "ms": res["prep_ms"],
                        "gates_per_s": res["prep_gates"] / (res["prep_ms"] * 1e-3) if res["prep_ms"] > 0 else None},
         "state": {"sum_n": res["sum_n"], "log_norm": res["log_norm"], "discarded": stats["discarded"], "svd_sweeps_max": stats["sweeps"],
-                  "svd_converged": stats["converged"]},
+                  "svd_converged": stats["converged"], "full_environment_readout": res["full"]},
         "cpu_baseline": cpu,
         "per_workload": per_workload,
     }

@@ -107,6 +107,14 @@ int u1mps_expect_n(u1mps_t* h, int site, double* out_host);        /* canonical-
 int u1mps_expect_n_all(u1mps_t* h, double* out_host /*[M]*/);      /* all sites, one launch */
 int u1mps_bond_entropy(u1mps_t* h, int bond, double* out_host);    /* -sum lambda^2 ln lambda^2 (natural log, S23) */
 int u1mps_bond_entropy_all(u1mps_t* h, double* out_host /*[M+1]*/);
+/* Full-environment <psi|n_k|psi> / <psi|psi> of all sites (state of Eq.15): left and
+ * right environments contracted explicitly, exact for whatever Gamma, lambda the handle holds - unlike the
+ * canonical-form u1mps_expect_n, which is exact only while nothing has been truncated (Eq.10).  The caller
+ * provides DEVICE scratch (256-byte aligned) of at least u1mps_expect_n_full_bytes (it depends on the current sector
+ * tables: all left environments of the chain are kept, sum over bonds and sectors of n^2 complex128, plus two Gamma-sized
+ * buffers); U1MPS_ENOMEM if it is too small.  out_host: [M].  Both [sync]. */
+int u1mps_expect_n_full_bytes(u1mps_t* h, size_t* bytes_host);
+int u1mps_expect_n_full(u1mps_t* h, double* out_host, void* scratch_dev, size_t scratch_bytes);
 /* Sector table of a bond: writes up to cap (charge, count) pairs, ascending charge; *n_sectors = how many exist. */
 int u1mps_bond_info(u1mps_t* h, int bond, int32_t* n_sectors, int32_t* charges, int32_t* counts, int cap);
 int u1mps_bond_dims(u1mps_t* h, int32_t* dims_host /*[M+1]*/);

@@ -22,7 +22,7 @@ EXPORTS = [
     "u1mps_bond_dims", "u1mps_last_stats", "u1mps_export_bond", "u1mps_export_site", "u1mps_import_bond",
     "u1mps_import_site", "u1mps_set_log_norm", "u1mps_staged_info", "u1mps_export_staged_theta",
     "u1mps_export_staged_svd", "u1mps_launch_count", "u1mps_profile_enable", "u1mps_profile_read",
-    "u1mps_stage_name", "u1mps_svd_trace", "u1mps_clear_status",
+    "u1mps_stage_name", "u1mps_svd_trace", "u1mps_clear_status", "u1mps_expect_n_full_bytes", "u1mps_expect_n_full",
 ]
 NSTAGE = 8
 
@@ -84,6 +84,8 @@ def load_library() -> C.CDLL:
     lib.u1mps_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
     lib.u1mps_svd_trace.argtypes = [vp, C.POINTER(C.c_longlong), C.c_int]
     lib.u1mps_clear_status.argtypes = [vp]
+    lib.u1mps_expect_n_full_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+    lib.u1mps_expect_n_full.argtypes = [vp, dp, vp, C.c_size_t]
     lib.u1mps_stage_name.restype = C.c_char_p
     lib.u1mps_stage_name.argtypes = [C.c_int]
     for name in EXPORTS:
@@ -206,6 +208,16 @@ class U1MPS:
     def expect_n_all(self) -> np.ndarray:
         out = np.zeros(self.M)
         self._ck(self.lib.u1mps_expect_n_all(self.h, _ptr(out, C.POINTER(C.c_double))))
+        return out
+
+    def expect_n_full(self) -> np.ndarray:
+        """<psi|n_k|psi> / <psi|psi> with explicit environments (exact also after truncation); scratch from torch."""
+        import torch
+        nbytes = C.c_size_t()
+        self._ck(self.lib.u1mps_expect_n_full_bytes(self.h, C.byref(nbytes)))
+        scratch = torch.empty(max(nbytes.value, 256), dtype=torch.uint8, device="cuda")
+        out = np.zeros(self.M)
+        self._ck(self.lib.u1mps_expect_n_full(self.h, _ptr(out, C.POINTER(C.c_double)), C.c_void_p(scratch.data_ptr()), nbytes.value))
         return out
 
     def bond_entropy(self, bond: int) -> float:

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libu1mps.so")
-SOURCES = ["api.cu", "plan.cu", "contract.cu", "svd.cu", "select.cu", "readout.cu"]
+SOURCES = ["api.cu", "plan.cu", "contract.cu", "svd.cu", "select.cu", "readout.cu", "envs.cu"]
 PROBE = os.path.join(HERE, "fp64_probe")          # measured FP64 peak (csrc/fp64_probe.cu), run by bench.py
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--extended-lambda",
          "-shared", "-Xcompiler", "-fPIC"]

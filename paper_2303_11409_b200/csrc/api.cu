@@ -433,6 +433,46 @@ int u1mps_expect_n(u1mps_t* h, int site, double* out) {
   return U1MPS_OK;
 }
 
+// tables and block offsets of the whole chain on the host (for the environment sweeps)
+static int env_tables(u1mps_t* h, std::vector<long long>& gamoff, std::vector<long long>& gused) {
+  int r = sync_tables(h);
+  if (r) return r;
+  gamoff.resize((size_t)h->M * h->NC * h->d);
+  CK(cudaMemcpyAsync(gamoff.data(), h->S.gamoff, gamoff.size() * 8, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  gused.assign(h->M, 0);
+  for (int s = 0; s < h->M; ++s)
+    for (int cl = 0; cl < h->NC; ++cl)
+      for (int i = 0; i < h->d && cl - i >= 0; ++i)
+        gused[s] += (long long)h->h_nb[(size_t)s * h->NC + cl] * h->h_nb[(size_t)(s + 1) * h->NC + cl - i];
+  return U1MPS_OK;
+}
+
+int u1mps_expect_n_full_bytes(u1mps_t* h, size_t* bytes) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
+  if (!h || !bytes) return U1MPS_EINVAL;
+  if (h->stage != ST_NONE) return U1MPS_ESTAGED;
+  std::vector<long long> gamoff, gused;
+  int r = env_tables(h, gamoff, gused);
+  if (r) return r;
+  *bytes = u1_env_scratch_bytes(h->M, h->NC, h->d, h->h_nb, gused);
+  return U1MPS_OK;
+}
+
+int u1mps_expect_n_full(u1mps_t* h, double* out, void* scratch_dev, size_t scratch_bytes) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
+  if (!h || !out || !scratch_dev || ((uintptr_t)scratch_dev & 255)) return U1MPS_EINVAL;
+  if (h->stage != ST_NONE) return U1MPS_ESTAGED;
+  std::vector<long long> gamoff, gused;
+  int r = env_tables(h, gamoff, gused);
+  if (r) return r;
+  if (scratch_bytes < u1_env_scratch_bytes(h->M, h->NC, h->d, h->h_nb, gused)) return U1MPS_ENOMEM;
+  CK(u1_env_expect_n(h->S, h->h_nb, gamoff, gused, scratch_dev, h->dout, h->L));
+  CK(cudaMemcpyAsync(out, h->dout, (size_t)h->M * 8, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return U1MPS_OK;
+}
+
 int u1mps_bond_entropy_all(u1mps_t* h, double* out) {
   if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out) return U1MPS_EINVAL;

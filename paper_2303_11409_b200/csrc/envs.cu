@@ -1,0 +1,357 @@
+// envs.cu — full-environment expectation values <psi|n_k|psi> / <psi|psi> of the U(1) MPS (SURVEY section 8(f)-4,
+// PAPER.md Eq.15 L112-114 for the state, Eq.10 L74-80 for what "canonical" would mean): once truncation has broken the
+// canonical form, the lambda-weighted formula of step a6 is only approximate, while the contraction with explicit left
+// and right environments is exact for whatever Gamma, lambda the state holds.
+//   A^[s](cl, cr) = Gamma^[s][cl, cr] diag(lambda^[s+1][cr])
+//   E_0 = {N: [[1]]},  E_{s+1}[cr] = sum_cl A^H E_s[cl] A          (left environments, n x n per sector)
+//   R_M = {0: [[1]]},  R_s[cl]     = sum_cr A R_{s+1}[cr] A^H      (right environments)
+//   <n_s> = sum_{cl,cr} (cl - cr) tr(A^H E_s[cl] A R_{s+1}[cr]) / E_M[0]
+// Everything is a grouped complex128 GEMM over the charge blocks of one site (FP64 DMMA tiles, as in step a2); the
+// trace is an element-wise inner product of T = E_s Gamma and S = Gamma lambda R lambda.  The host knows the sector
+// tables (the call synchronises anyway), builds the block descriptors of all stages once and uploads them; the device
+// does all arithmetic.
+#include <algorithm>
+#include <vector>
+#include "common.cuh"
+
+#define EV_THREADS 128
+#define EV_KC 16
+#define EV_LD 34
+#define EV_MAXTERM 8   // = U1MPS_D_MAX: a block sum runs over at most d occupations
+
+struct EnvDesc {
+  const cplx* A[EV_MAXTERM];     // term t: left operand, dense row-major (m x k, or k x m if opA)
+  const cplx* B[EV_MAXTERM];     // ... right operand (k x n, or n x k if opB)
+  const double* ks[EV_MAXTERM];  // ... optional scale over the inner index (nullptr: none)
+  int k[EV_MAXTERM];
+  cplx* C;                       // m x n row-major
+  const double* rs;              // optional output row / column scales
+  const double* cs;
+  double alpha;
+  int m, n, nterm, opA, opB;     // op = 1: the operand is the conjugate transpose of what is stored
+};
+
+// C = alpha diag(rs) (sum_t op(A_t) diag(ks_t) op(B_t)) diag(cs), 32 x 32 output tiles, K-chunks of 16 through shared
+// memory, 4 warps x one 8-row strip each, DMMA.8x8x4 (4 real products per complex one).
+__global__ void __launch_bounds__(EV_THREADS) env_gemm_kernel(const EnvDesc* __restrict__ desc, const int* __restrict__ tpref, int ndesc) {
+  __shared__ __align__(16) cplx As[EV_KC * EV_LD];   // As[kk][a]
+  __shared__ __align__(16) cplx Bs[EV_KC * EV_LD];   // Bs[kk][b]
+  const int total = tpref[ndesc];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, lr = lane >> 2, lk = lane & 3;
+  for (int tile = blockIdx.x; tile < total; tile += gridDim.x) {
+    int lo = 0, hi = ndesc;
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (tpref[mid] <= tile) lo = mid; else hi = mid; }
+    const EnvDesc& D = desc[lo];
+    const int m = D.m, n = D.n, tcols = u1_ceil_div(n, U1_TILE), local = tile - tpref[lo];
+    const int a0 = (local / tcols) * U1_TILE, b0 = (local % tcols) * U1_TILE;
+    double cre[4][2], cim[4][2];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { cre[u][0] = cre[u][1] = 0.0; cim[u][0] = cim[u][1] = 0.0; }
+    for (int t = 0; t < D.nterm; ++t) {
+      const cplx* A = D.A[t];
+      const cplx* B = D.B[t];
+      const double* ks = D.ks[t];
+      const int K = D.k[t];
+      for (int k0 = 0; k0 < K; k0 += EV_KC) {
+        cplx ra[4], rb[4];
+        // A chunk: 32 (a) x 16 (kk)
+        if (!D.opA) {   // stored m x K: kk fastest
+          const int kk = tid & (EV_KC - 1);
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const int a = (tid >> 4) + 8 * x;
+            cplx v = make_double2(0.0, 0.0);
+            if (a0 + a < m && k0 + kk < K) v = A[(long long)(a0 + a) * K + k0 + kk];
+            if (ks && k0 + kk < K) { const double sc = ks[k0 + kk]; v.x *= sc; v.y *= sc; }
+            ra[x] = v;
+          }
+        } else {        // stored K x m, conjugated: a fastest
+          const int a = tid & (U1_TILE - 1);
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const int kk = (tid >> 5) + 4 * x;
+            cplx v = make_double2(0.0, 0.0);
+            if (a0 + a < m && k0 + kk < K) { v = A[(long long)(k0 + kk) * m + a0 + a]; v.y = -v.y; }
+            if (ks && k0 + kk < K) { const double sc = ks[k0 + kk]; v.x *= sc; v.y *= sc; }
+            ra[x] = v;
+          }
+        }
+        // B chunk: 16 (kk) x 32 (b)
+        if (!D.opB) {   // stored K x n: b fastest
+          const int b = tid & (U1_TILE - 1);
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const int kk = (tid >> 5) + 4 * x;
+            cplx v = make_double2(0.0, 0.0);
+            if (b0 + b < n && k0 + kk < K) v = B[(long long)(k0 + kk) * n + b0 + b];
+            rb[x] = v;
+          }
+        } else {        // stored n x K, conjugated: kk fastest
+          const int kk = tid & (EV_KC - 1);
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const int b = (tid >> 4) + 8 * x;
+            cplx v = make_double2(0.0, 0.0);
+            if (b0 + b < n && k0 + kk < K) { v = B[(long long)(b0 + b) * K + k0 + kk]; v.y = -v.y; }
+            rb[x] = v;
+          }
+        }
+        __syncthreads();  // the previous chunk has been consumed
+#pragma unroll
+        for (int x = 0; x < 4; ++x) {
+          if (!D.opA) As[(tid & (EV_KC - 1)) * EV_LD + (tid >> 4) + 8 * x] = ra[x];
+          else As[((tid >> 5) + 4 * x) * EV_LD + (tid & (U1_TILE - 1))] = ra[x];
+          if (!D.opB) Bs[((tid >> 5) + 4 * x) * EV_LD + (tid & (U1_TILE - 1))] = rb[x];
+          else Bs[(tid & (EV_KC - 1)) * EV_LD + (tid >> 4) + 8 * x] = rb[x];
+        }
+        __syncthreads();
+        const int nk = (min(EV_KC, K - k0) + 3) >> 2;
+        for (int kq = 0; kq < nk; ++kq) {
+          const cplx av = As[(4 * kq + lk) * EV_LD + 8 * warp + lr];
+          const double nai = -av.y;
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const cplx bv = Bs[(4 * kq + lk) * EV_LD + 8 * u + lr];
+            dmma(cre[u][0], cre[u][1], av.x, bv.x); dmma(cre[u][0], cre[u][1], nai, bv.y);
+            dmma(cim[u][0], cim[u][1], av.x, bv.y); dmma(cim[u][0], cim[u][1], av.y, bv.x);
+          }
+        }
+      }
+    }
+    __syncthreads();  // before the next tile refills the stages
+    const int a = a0 + 8 * warp + lr;
+    if (a < m) {
+      const double ra_ = D.alpha * (D.rs ? D.rs[a] : 1.0);
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int x = 0; x < 2; ++x) {
+          const int b = b0 + 8 * u + 2 * lk + x;
+          if (b < n) {
+            const double sc = ra_ * (D.cs ? D.cs[b] : 1.0);
+            D.C[(long long)a * n + b] = make_double2(cre[u][x] * sc, cim[u][x] * sc);
+          }
+        }
+    }
+  }
+}
+
+// Re sum_e T[e] conj(S[e]) over [0, len): K slices, lanes / warps / slices summed in a fixed order (the last CTA adds
+// the slice sums), so the result does not depend on timing.
+#define EV_DOT_THREADS 256
+#define EV_DOT_SLICES 128
+__global__ void __launch_bounds__(EV_DOT_THREADS) env_dot_kernel(const cplx* __restrict__ T, const cplx* __restrict__ Sb, long long len,
+                                                                 double* part, int* count, double* out) {
+  __shared__ double red[EV_DOT_THREADS / 32];
+  __shared__ int s_last;
+  const int tid = threadIdx.x, K = gridDim.x, j = blockIdx.x;
+  const long long e0 = len * j / K, e1 = len * (j + 1) / K;
+  double acc = 0.0;
+  for (long long e = e0 + tid; e < e1; e += EV_DOT_THREADS) {
+    const cplx t = T[e], s = Sb[e];
+    acc = fma(t.x, s.x, fma(t.y, s.y, acc));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if ((tid & 31) == 0) red[tid >> 5] = acc;
+  __syncthreads();
+  if (tid == 0) {
+    double t = 0.0;
+    for (int w = 0; w < EV_DOT_THREADS / 32; ++w) t += red[w];
+    part[j] = t;
+    __threadfence();
+    s_last = (atomicAdd(count, 1) == K - 1) ? 1 : 0;
+  }
+  __syncthreads();
+  if (s_last && tid == 0) {
+    __threadfence();
+    double t = 0.0;
+    for (int jj = 0; jj < K; ++jj) t += __ldcg(&part[jj]);
+    *out = t;
+    *count = 0;
+  }
+}
+
+// <n_s> = (sum over blocks of (cl - cr) tr(...)) / <psi|psi>,  <psi|psi> = E_M[0]
+__global__ void env_finish_kernel(double* out, int M, const cplx* norm) {
+  const double inv = 1.0 / norm->x;
+  for (int s = threadIdx.x; s < M; s += blockDim.x) out[s] *= inv;
+}
+
+namespace {
+inline size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct EnvLayout {
+  std::vector<long long> Ebase;   // [M+1] element offset of the environments of bond k inside the E store
+  std::vector<long long> eoff;    // [(M+1)*NC] offset of sector c inside bond k's environments
+  long long Etot = 0, maxE = 0, maxG = 0;
+  size_t ndesc = 0, npref = 0;    // descriptors and tile-prefix entries of all launches
+  size_t o_desc = 0, o_pref = 0, o_E = 0, o_R = 0, o_T = 0, o_S = 0, o_misc = 0, total = 0;
+};
+
+EnvLayout env_layout(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused) {
+  EnvLayout Y;
+  Y.Ebase.resize(M + 1); Y.eoff.assign((size_t)(M + 1) * NC, 0);
+  for (int k = 0; k <= M; ++k) {
+    Y.Ebase[k] = Y.Etot;
+    long long run = 0;
+    for (int c = 0; c < NC; ++c) { Y.eoff[(size_t)k * NC + c] = run; const long long n = nb[(size_t)k * NC + c]; run += n * n; }
+    Y.Etot += run;
+    Y.maxE = std::max(Y.maxE, run);
+  }
+  for (int s = 0; s < M; ++s) {
+    Y.maxG = std::max(Y.maxG, gused[s]);
+    size_t nblk = 0, nblk1 = 0, nL = 0, nR = 0;
+    for (int cl = 0; cl < NC; ++cl) {
+      if (nb[(size_t)s * NC + cl]) ++nL;
+      if (nb[(size_t)(s + 1) * NC + cl]) ++nR;
+      for (int i = 0; i < d && cl - i >= 0; ++i)
+        if (nb[(size_t)s * NC + cl] && nb[(size_t)(s + 1) * NC + cl - i]) { ++nblk; if (i) ++nblk1; }
+    }
+    // launches of a site: L1 (blocks), L2 (right sectors), R1 (blocks), TT (blocks with i >= 1), R2 (left sectors)
+    Y.ndesc += 2 * nblk + nblk1 + nL + nR;
+    Y.npref += 2 * nblk + nblk1 + nL + nR + 5;
+  }
+  size_t o = 0;
+  Y.o_desc = o; o = al256(o + Y.ndesc * sizeof(EnvDesc));
+  Y.o_pref = o; o = al256(o + Y.npref * sizeof(int));
+  Y.o_E = o;    o = al256(o + (size_t)Y.Etot * sizeof(cplx));
+  Y.o_R = o;    o = al256(o + (size_t)2 * Y.maxE * sizeof(cplx));
+  Y.o_T = o;    o = al256(o + (size_t)Y.maxG * sizeof(cplx));
+  Y.o_S = o;    o = al256(o + (size_t)Y.maxG * sizeof(cplx));
+  Y.o_misc = o; o = al256(o + (EV_DOT_SLICES + 8) * sizeof(double));
+  Y.total = o;
+  return Y;
+}
+}  // namespace
+
+size_t u1_env_scratch_bytes(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused) {
+  return env_layout(M, NC, d, nb, gused).total;
+}
+
+// Host driver: descriptors of all stages from the sector tables, one upload, then the two sweeps.
+// nb: [(M+1)*NC] sector sizes; gamoff: [M*NC*d] block offsets of every site; gused: [M] elements used per site.
+cudaError_t u1_env_expect_n(const DevState& S, const std::vector<int>& nb, const std::vector<long long>& gamoff,
+                            const std::vector<long long>& gused, void* scratch, double* out_dev, const LaunchCfg& L) {
+  const int M = S.M, NC = S.NC, d = S.d;
+  const EnvLayout Y = env_layout(M, NC, d, nb, gused);
+  char* base = (char*)scratch;
+  EnvDesc* d_desc = (EnvDesc*)(base + Y.o_desc);
+  int* d_pref = (int*)(base + Y.o_pref);
+  cplx* Ebuf = (cplx*)(base + Y.o_E);
+  cplx* Rbuf = (cplx*)(base + Y.o_R);
+  cplx* Tbuf = (cplx*)(base + Y.o_T);
+  cplx* Sbuf = (cplx*)(base + Y.o_S);
+  double* part = (double*)(base + Y.o_misc);
+  int* count = (int*)(part + EV_DOT_SLICES);
+  // offsets of the sectors inside lambda^[k]
+  std::vector<int> ob((size_t)(M + 1) * NC);
+  for (int k = 0; k <= M; ++k) { int run = 0; for (int c = 0; c < NC; ++c) { ob[(size_t)k * NC + c] = run; run += nb[(size_t)k * NC + c]; } }
+  auto nK = [&](int k, int c) { return nb[(size_t)k * NC + c]; };
+  auto Eptr = [&](int k, int c) { return Ebuf + Y.Ebase[k] + Y.eoff[(size_t)k * NC + c]; };
+  auto Rptr = [&](int k, int c) { return Rbuf + (size_t)(k & 1) * Y.maxE + Y.eoff[(size_t)k * NC + c]; };
+  auto lamp = [&](int k, int c) { return S.lam + (size_t)k * S.chi + ob[(size_t)k * NC + c]; };
+  auto goff = [&](int s, int cl, int i) { return gamoff[((size_t)s * NC + cl) * d + i]; };
+
+  struct Launch { size_t d0, p0; int nd, tiles; };
+  std::vector<EnvDesc> descs; descs.reserve(Y.ndesc);
+  std::vector<int> prefs; prefs.reserve(Y.npref);
+  std::vector<Launch> LA((size_t)M * 5);   // per site: L1, L2, R1, TT, R2
+  auto begin_launch = [&](Launch& la) { la.d0 = descs.size(); la.p0 = prefs.size(); la.nd = 0; la.tiles = 0; prefs.push_back(0); };
+  auto push = [&](Launch& la, const EnvDesc& D) {
+    descs.push_back(D);
+    la.tiles += u1_ceil_div(D.m, U1_TILE) * u1_ceil_div(D.n, U1_TILE);
+    prefs.push_back(la.tiles);
+    ++la.nd;
+  };
+  EnvDesc Z;
+  for (int t = 0; t < EV_MAXTERM; ++t) { Z.A[t] = nullptr; Z.B[t] = nullptr; Z.ks[t] = nullptr; Z.k[t] = 0; }
+  Z.C = nullptr; Z.rs = nullptr; Z.cs = nullptr; Z.alpha = 1.0; Z.m = Z.n = Z.nterm = Z.opA = Z.opB = 0;
+  for (int s = 0; s < M; ++s) {
+    const cplx* G = S.gam + (size_t)s * S.gcap;
+    Launch &l1 = LA[(size_t)s * 5], &l2 = LA[(size_t)s * 5 + 1], &r1 = LA[(size_t)s * 5 + 2], &tt = LA[(size_t)s * 5 + 3], &r2 = LA[(size_t)s * 5 + 4];
+    // L1: T_f = E_s[cl] Gamma_f            TT: the same, times the occupation i (only i >= 1)
+    begin_launch(l1);
+    for (int cl = 0; cl < NC; ++cl) for (int i = 0; i < d && cl - i >= 0; ++i) {
+      const int nl = nK(s, cl), nr = nK(s + 1, cl - i);
+      if (!nl || !nr) continue;
+      EnvDesc D = Z; D.m = nl; D.n = nr; D.nterm = 1; D.A[0] = Eptr(s, cl); D.B[0] = G + goff(s, cl, i); D.k[0] = nl; D.C = Tbuf + goff(s, cl, i);
+      push(l1, D);
+    }
+    begin_launch(tt);
+    for (int cl = 0; cl < NC; ++cl) for (int i = 1; i < d && cl - i >= 0; ++i) {
+      const int nl = nK(s, cl), nr = nK(s + 1, cl - i);
+      if (!nl || !nr) continue;
+      EnvDesc D = Z; D.m = nl; D.n = nr; D.nterm = 1; D.A[0] = Eptr(s, cl); D.B[0] = G + goff(s, cl, i); D.k[0] = nl; D.C = Tbuf + goff(s, cl, i);
+      D.alpha = (double)i;
+      push(tt, D);
+    }
+    // L2: E_{s+1}[cr] = lam (sum_i Gamma_f^H T_f) lam
+    begin_launch(l2);
+    for (int cr = 0; cr < NC; ++cr) {
+      const int nr = nK(s + 1, cr);
+      if (!nr) continue;
+      EnvDesc D = Z; D.m = nr; D.n = nr; D.opA = 1; D.C = Eptr(s + 1, cr); D.rs = lamp(s + 1, cr); D.cs = lamp(s + 1, cr);
+      for (int i = 0; i < d && cr + i < NC; ++i) {
+        const int nl = nK(s, cr + i);
+        if (!nl) continue;
+        D.A[D.nterm] = G + goff(s, cr + i, i); D.B[D.nterm] = Tbuf + goff(s, cr + i, i); D.k[D.nterm] = nl; ++D.nterm;
+      }
+      push(l2, D);   // (no term: a sector no block reaches - its environment is zero, and is written as such)
+    }
+    // R1: S_f = Gamma_f lam R_{s+1}[cr] lam
+    begin_launch(r1);
+    for (int cl = 0; cl < NC; ++cl) for (int i = 0; i < d && cl - i >= 0; ++i) {
+      const int nl = nK(s, cl), nr = nK(s + 1, cl - i);
+      if (!nl || !nr) continue;
+      EnvDesc D = Z; D.m = nl; D.n = nr; D.nterm = 1; D.A[0] = G + goff(s, cl, i); D.ks[0] = lamp(s + 1, cl - i); D.B[0] = Rptr(s + 1, cl - i);
+      D.k[0] = nr; D.cs = lamp(s + 1, cl - i); D.C = Sbuf + goff(s, cl, i);
+      push(r1, D);
+    }
+    // R2: R_s[cl] = sum_i S_f Gamma_f^H
+    begin_launch(r2);
+    for (int cl = 0; cl < NC; ++cl) {
+      const int nl = nK(s, cl);
+      if (!nl) continue;
+      EnvDesc D = Z; D.m = nl; D.n = nl; D.opB = 1; D.C = Rptr(s, cl);
+      for (int i = 0; i < d && cl - i >= 0; ++i) {
+        const int nr = nK(s + 1, cl - i);
+        if (!nr) continue;
+        D.A[D.nterm] = Sbuf + goff(s, cl, i); D.B[D.nterm] = G + goff(s, cl, i); D.k[D.nterm] = nr; ++D.nterm;
+      }
+      push(r2, D);   // (no term: a dead-end sector, left behind by a truncation - zero environment)
+    }
+  }
+  cudaError_t err;
+  if ((err = cudaMemcpyAsync(d_desc, descs.data(), descs.size() * sizeof(EnvDesc), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemcpyAsync(d_pref, prefs.data(), prefs.size() * sizeof(int), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemsetAsync(Ebuf, 0, (size_t)Y.Etot * sizeof(cplx), L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemsetAsync(Rbuf, 0, (size_t)2 * Y.maxE * sizeof(cplx), L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemsetAsync(part, 0, (EV_DOT_SLICES + 8) * sizeof(double), L.stream)) != cudaSuccess) return err;
+  const cplx one = make_double2(1.0, 0.0);
+  if ((err = cudaMemcpyAsync(Eptr(0, S.N), &one, sizeof(cplx), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemcpyAsync(Rptr(M, 0), &one, sizeof(cplx), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  // the host vectors must outlive the asynchronous copies out of pageable memory: those are staged by the runtime before
+  // the call returns, so nothing more is needed here
+  auto run = [&](const Launch& la) {
+    if (la.tiles == 0) return;
+    L.prof->begin(U1_ST_READOUT, L.stream);
+    env_gemm_kernel<<<std::min(la.tiles, L.sms * 8), EV_THREADS, 0, L.stream>>>(d_desc + la.d0, d_pref + la.p0, la.nd);
+    L.prof->end(L.stream);
+    ++*L.launches;
+  };
+  for (int s = 0; s < M; ++s) { run(LA[(size_t)s * 5]); run(LA[(size_t)s * 5 + 1]); }
+  for (int s = M - 1; s >= 0; --s) {
+    run(LA[(size_t)s * 5 + 2]);
+    if ((err = cudaMemsetAsync(Tbuf, 0, (size_t)gused[s] * sizeof(cplx), L.stream)) != cudaSuccess) return err;
+    run(LA[(size_t)s * 5 + 3]);
+    L.prof->begin(U1_ST_READOUT, L.stream);
+    env_dot_kernel<<<EV_DOT_SLICES, EV_DOT_THREADS, 0, L.stream>>>(Tbuf, Sbuf, gused[s], part, count, out_dev + s);
+    L.prof->end(L.stream);
+    ++*L.launches;
+    run(LA[(size_t)s * 5 + 4]);
+  }
+  env_finish_kernel<<<1, 256, 0, L.stream>>>(out_dev, M, Eptr(M, 0));
+  ++*L.launches;
+  return cudaGetLastError();
+}

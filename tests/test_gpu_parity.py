@@ -170,6 +170,32 @@ def test_config5_trajectory_states_teacher_forced():
     _teacher_forced_on_trajectory(5, [(10, 7), (11, 3)], max_ties=10)
 
 
+# ------------------------------------------------------------------ full-environment read-out
+@pytest.mark.parametrize("idx,M,N,chi,cols", [
+    (2, 16, 8, 12, 14),     # hard truncation: the canonical form is badly broken
+    (3, 20, 10, 6, 40),
+    (4, 8, 4, 6, 8),        # d = 5: sums over up to five occupations per sector
+    (5, 10, 5, 6, 10),
+])
+def test_expect_n_full_on_truncated_states(idx, M, N, chi, cols):
+    """u1mps_expect_n_full = <psi|n_k|psi>/<psi|psi> with explicit environments against the oracle's expect_n_full
+    (pinned by P10 against the state vector) on states whose canonical form truncation has broken: 1e-9 per site, and
+    sum_k = N to 1e-9 (charge conservation, Eq.1) - which the canonical-form read-out misses by far more."""
+    w = inputs.small_variant(inputs.WORKLOADS[idx], M=M, N=N, chi=chi, columns=cols)
+    ora, gpu = run_both(w)
+    assert_observables(ora, gpu)
+    want = np.array([ora.expect_n_full(s) for s in range(w.M)])
+    got = gpu.expect_n_full()
+    assert np.max(np.abs(got - want)) <= 1e-9, np.max(np.abs(got - want))
+    assert abs(np.sum(got) - w.N) <= 1e-9
+    assert ora.discarded_total > 1e-9                                   # truncation did happen
+    assert np.array_equal(got, gpu.expect_n_full())                     # deterministic reductions
+    # untruncated product state: both read-outs agree exactly
+    fresh = make_gpu(w.M, w.d, w.N, w.chi)
+    fresh.set_product_state(w.occ)
+    assert np.allclose(fresh.expect_n_full(), w.occ, atol=1e-15)
+
+
 # ------------------------------------------------------------------ the tie order at the cut (reading S8)
 def test_exact_tie_at_the_cut_and_keep_at_least_one():
     """An exact tie across two sectors at the cut: |10> under a gate with equal amplitudes to stay and to hop gives
