@@ -71,6 +71,34 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
+// Trial build -DSV_TMA (profiles/r2_tma_trial.md): the chunk loader as 1-D bulk copies (cp.async.bulk, the TMA engine,
+// completion on an mbarrier per ring stage) issued by one warp, instead of 16-byte cp.async by all threads.
+struct RingState {
+#ifdef SV_TMA
+  unsigned long long* bar;   // [SV_NSTAGE] mbarriers in shared memory
+  unsigned phase;            // bit s: parity the next wait on stage s expects
+#endif
+};
+#ifdef SV_TMA
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
+  unsigned ok = 0;
+  for (unsigned spins = 0; !ok && spins < (1u << 22); ++spins)   // bounded: a lost completion must not hang the GPU
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+}
+#endif
+
 // Named barrier of a 128-thread group (id g + 1; 0 is __syncthreads) and its group-wide OR.
 __device__ __forceinline__ void gsync(int g) { asm volatile("bar.sync %0, 128;\n" ::"r"(g + 1) : "memory"); }
 __device__ __forceinline__ int gsync_or(int g, int pred) {
@@ -109,6 +137,31 @@ __device__ __forceinline__ Loader make_loader(const Item& I, int gtid) {
   }
   return L;
 }
+#ifdef SV_TMA
+// stage `sidx`: one bulk copy per present column (32 rows x 16 B = 512 B contiguous in global and in shared memory),
+// lane j of warp 0 takes column j; ragged tails and absent columns are zero-filled with ordinary stores
+__device__ __forceinline__ void load_chunk_tma(cplx* st, int ld, const Item& I, int row0, int rowlim, int gtid, RingState& RS, int sidx) {
+  const int rows = min(SV_R, rowlim - row0);
+  const int lane = gtid & 31;
+  if (gtid < 32) {
+    const bool present = lane < U1_PB ? lane < I.na : lane - U1_PB < I.nb;
+    const unsigned bytes = present ? (unsigned)rows * 16u : 0u;
+    unsigned total = bytes;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
+    if (lane == 0) mbar_expect_tx(RS.bar + sidx, total);
+    __syncwarp();
+    if (present) bulk_g2s(st + lane * ld, I.W + (long long)I.col[lane] * I.mt + row0, bytes, RS.bar + sidx);
+  }
+  if (rows < SV_R || I.na < U1_PB || I.nb < U1_PB) {
+    for (int idx = gtid; idx < SV_W * SV_R; idx += SV_GROUP) {
+      const int j = idx / SV_R, r = idx - j * SV_R;
+      const bool present = j < U1_PB ? j < I.na : j - U1_PB < I.nb;
+      if (!present || r >= rows) st[j * ld + r] = make_double2(0.0, 0.0);
+    }
+  }
+}
+#endif
 __device__ __forceinline__ void load_chunk(cplx* st, int ld, const Loader& L, int row0, int rowlim, int gtid) {
   const int r = gtid & (SV_R - 1);
   const bool rok = row0 + r < rowlim;
@@ -123,7 +176,7 @@ __device__ __forceinline__ void load_chunk(cplx* st, int ld, const Loader& L, in
 // ---- phase 1: H = P^H P over rows [0, m).  H is Hermitian: only the 10 tiles (8 x 8 each) of the upper triangle of
 // the 4 x 4 tile grid are computed, 3 + 3 + 2 + 2 per warp: warp 0 (0,0) (0,1) (0,2); warp 1 (3,0) (3,1) (3,2), stored
 // as the conjugate transposes (0,3) (1,3) (2,3); warp 2 (1,1) (1,2); warp 3 (2,2) (3,3).
-__device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I, const Loader& L, int g, int gtid) {
+__device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I, const Loader& L, RingState& RS, int g, int gtid) {
   const int lane = gtid & 31, warp = gtid >> 5;
   const int lr = lane >> 2, lk = lane & 3;
   // tile slots of this warp: (ta[u], tb[u]), u < nt
@@ -139,17 +192,33 @@ __device__ __forceinline__ void gram_phase(cplx* stages, cplx* Hs, const Item& I
 #pragma unroll
   for (int u = 0; u < 3; ++u) { t1[u][0] = t1[u][1] = 0.0; t2[u][0] = t2[u][1] = 0.0; t3[u][0] = t3[u][1] = 0.0; }
   const int nch = (I.m + SV_R - 1) / SV_R;
+#ifdef SV_TMA
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // ordinary writes to the ring (H, Qt of the last item) before bulk writes
+  gsync(g);
+#endif
 #pragma unroll
   for (int p = 0; p < SV_NSTAGE - 1; ++p) {
+#ifdef SV_TMA
+    if (p < nch) load_chunk_tma(stages + p * SV_STAGE, SV_LDG, I, p * SV_R, I.m, gtid, RS, p);
+#else
     if (p < nch) load_chunk(stages + p * SV_STAGE, SV_LDG, L, p * SV_R, I.m, gtid);
     cp_async_commit();
+#endif
   }
   for (int c = 0; c < nch; ++c) {
+#ifdef SV_TMA
+    mbar_wait(RS.bar + c % SV_NSTAGE, (RS.phase >> (c % SV_NSTAGE)) & 1u);
+    RS.phase ^= 1u << (c % SV_NSTAGE);
+    gsync(g);  // everybody is done with chunk c - 1 (and sees the zero fill of chunk c): its stage may be refilled
+    if (c + SV_NSTAGE - 1 < nch)
+      load_chunk_tma(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDG, I, (c + SV_NSTAGE - 1) * SV_R, I.m, gtid, RS, (c + SV_NSTAGE - 1) % SV_NSTAGE);
+#else
     cp_async_wait<SV_NSTAGE - 2>();
     gsync(g);  // chunk c has landed for everybody, and everybody is done with chunk c - 1: its stage may be refilled
     if (c + SV_NSTAGE - 1 < nch)
       load_chunk(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDG, L, (c + SV_NSTAGE - 1) * SV_R, I.m, gtid);
     cp_async_commit();
+#endif
     const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE + lr * SV_LDG + lk;
     const int rows = min(SV_R, I.m - c * SV_R);
     const int nk = (rows + 3) >> 2;
@@ -426,7 +495,7 @@ __device__ __forceinline__ void evd_phase(cplx* H, cplx* Qt, double4* Rm, uchar2
 
 // ---- phase 3: [Pa Pb] <- [Pa Pb] Q over all mt rows.  Warp w owns tile column w (8 columns) and all row tiles
 // of each 32-row chunk; its 32 x 8 slice of Q lives in registers as 8 B fragments.
-__device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const Item& I, const Loader& L, int g, int gtid) {
+__device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const Item& I, const Loader& L, RingState& RS, int g, int gtid) {
   const int lane = gtid & 31, warp = gtid >> 5;
   const int tj = warp;
   const int lr = lane >> 2, lk = lane & 3;
@@ -437,6 +506,9 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
     const cplx v = Qt[(8 * tj + lr) * SV_QLD + 4 * ks + lk];   // Q[k][j], k = 4 ks + lk, j = 8 tj + lr
     bre[ks] = v.x; bim[ks] = v.y; bsm[ks] = v.x + v.y;
   }
+#ifdef SV_TMA
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+#endif
   gsync(g);  // Q (aliased onto the ring) is in registers everywhere: the ring may be refilled
   // the two output columns of this lane
   long long gcol[2]; bool cok[2];
@@ -449,15 +521,27 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
   const int nch = (I.mt + SV_R - 1) / SV_R;
 #pragma unroll
   for (int p = 0; p < SV_NSTAGE - 1; ++p) {
+#ifdef SV_TMA
+    if (p < nch) load_chunk_tma(stages + p * SV_STAGE, SV_LDU, I, p * SV_R, I.mt, gtid, RS, p);
+#else
     if (p < nch) load_chunk(stages + p * SV_STAGE, SV_LDU, L, p * SV_R, I.mt, gtid);
     cp_async_commit();
+#endif
   }
   for (int c = 0; c < nch; ++c) {
+#ifdef SV_TMA
+    mbar_wait(RS.bar + c % SV_NSTAGE, (RS.phase >> (c % SV_NSTAGE)) & 1u);
+    RS.phase ^= 1u << (c % SV_NSTAGE);
+    gsync(g);  // everybody is done with chunk c - 1 (and sees the zero fill of chunk c): its stage may be refilled
+    if (c + SV_NSTAGE - 1 < nch)
+      load_chunk_tma(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDU, I, (c + SV_NSTAGE - 1) * SV_R, I.mt, gtid, RS, (c + SV_NSTAGE - 1) % SV_NSTAGE);
+#else
     cp_async_wait<SV_NSTAGE - 2>();
     gsync(g);  // chunk c has landed for everybody, and everybody is done with chunk c - 1: its stage may be refilled
     if (c + SV_NSTAGE - 1 < nch)
       load_chunk(stages + ((c + SV_NSTAGE - 1) % SV_NSTAGE) * SV_STAGE, SV_LDU, L, (c + SV_NSTAGE - 1) * SV_R, I.mt, gtid);
     cp_async_commit();
+#endif
     const cplx* st = stages + (c % SV_NSTAGE) * SV_STAGE;
     const int row0 = c * SV_R;
     const int rows = min(SV_R, I.mt - row0);
@@ -489,7 +573,7 @@ __device__ __forceinline__ void update_phase(cplx* stages, const cplx* Qt, const
 // negative if the limit was hit.  (A kernel of its own, svd_solo_kernel, launched in front of svd_kernel: it returns at
 // once unless the launch consists of such sectors only, and svd_kernel then finds every sector finished.)
 __device__ __forceinline__ int solo_sector(const Plan& P, int e, cplx* stages, cplx* Hs, cplx* Qs, double4* Rm, uchar2* tab, int* s_col,
-                                        int inner_max, int R) {
+                                        int inner_max, int R, RingState& RS) {
   const int gtid = threadIdx.x, g = 0;
   Item I;
   const int r = P.rows[e], q = P.cols[e], n = min(r, q);
@@ -509,7 +593,7 @@ __device__ __forceinline__ int solo_sector(const Plan& P, int e, cplx* stages, c
   gsync(g);
   const Loader L = make_loader(I, gtid);
   for (int iter = 0; iter < U1_MAXSWEEP; ++iter) {
-    gram_phase(stages, Hs, I, L, g, gtid);
+    gram_phase(stages, Hs, I, L, RS, g, gtid);
     int todo = 0, big = 0;
     for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
       const int p = idx >> 5, qq = idx & 31;
@@ -530,7 +614,7 @@ __device__ __forceinline__ int solo_sector(const Plan& P, int e, cplx* stages, c
     int inner = 0;
     evd_phase(Hs, Qs, Rm, tab, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max + 4, 0.0, g, gtid);
     __syncthreads();
-    update_phase(stages, Qs, I, L, g, gtid);
+    update_phase(stages, Qs, I, L, RS, g, gtid);
     __syncthreads();   // the update's stores are visible to the CTA's next Gram pass
     if (gtid == 0) {
       const int sw = min(iter, U1_MAXSWEEP - 1);
@@ -568,6 +652,16 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
   double4* Rm = reinterpret_cast<double4*>(Qs + SV_W * SV_QLD);   // [2][16] rotations of the current and the previous EVD round
   uchar2* tab = reinterpret_cast<uchar2*>(Rm + 2 * U1_PB);         // [32][16] pivots of the modulus ordering
   const int nblk = P.cnt[0], npair = P.cnt[1], maxP = P.cnt[3];
+  RingState RS;
+#ifdef SV_TMA
+  __shared__ __align__(8) unsigned long long s_bar[SV_NSTAGE];
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < SV_NSTAGE; ++i) mbar_init(&s_bar[i], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  RS.bar = s_bar; RS.phase = 0;
+  __syncthreads();
+#endif
   const int R = max(maxP, 1);                      // rounds of one cycle of the largest sector (= a "sweep" of the trace)
   const int E = G * S.NC;
   int* last_rot = P.flags;                         // [E] round after the last rotation outside the quadratic regime
@@ -673,7 +767,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
         gsync(g);
         SV_TICK(0);
         L = make_loader(I, gtid);
-        gram_phase(stages, Hs, I, L, g, gtid);
+        gram_phase(stages, Hs, I, L, RS, g, gtid);
         SV_TICK(1);
         // quick test, same entries and arithmetic as the rotations: anything to do?
         for (int idx = gtid; idx < SV_W * SV_W; idx += SV_GROUP) {
@@ -700,7 +794,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_kernel(DevState S
       if (todo) evd_phase(Hs, Qs, Rm, tab, I.nb > 0 ? U1_PB : U1_PB / 2, I.tol2, &inner, inner_max, SV_QUAD, g, gtid);
       __syncthreads();
       SV_TICK(2);
-      if (todo) update_phase(stages, Qs, I, L, g, gtid);
+      if (todo) update_phase(stages, Qs, I, L, RS, g, gtid);
       SV_TICK(3);
       // done: publish (the update's stores and the stamp before the counter)
       __syncthreads();
@@ -761,6 +855,17 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_solo_kernel(Plan 
   __shared__ int s_col[SV_W];
   const int nblk = P.cnt[0], maxP = P.cnt[3];
   if (maxP > 2 || nblk == 0) return;
+  RingState RS;
+#ifdef SV_TMA
+  __shared__ __align__(8) unsigned long long s_bar[SV_NSTAGE];
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < SV_NSTAGE; ++i) mbar_init(&s_bar[i], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  RS.bar = s_bar; RS.phase = 0;
+  __syncthreads();
+#endif
+
   cplx* stages = reinterpret_cast<cplx*>(smraw);
   cplx* Hs = stages;
   cplx* Qs = Hs + SV_W * SV_HLD;
@@ -771,7 +876,7 @@ __global__ void __launch_bounds__(U1_SVD_THREADS, SV_CTAS) svd_solo_kernel(Plan 
   for (int bi = blockIdx.x; bi < nblk; bi += gridDim.x) {
     const int e = P.blk[bi];
     __syncthreads();
-    const int visits = solo_sector(P, e, stages, Hs, Qs, Rm, tab, s_col, inner_max, R);
+    const int visits = solo_sector(P, e, stages, Hs, Qs, Rm, tab, s_col, inner_max, R, RS);
     __syncthreads();
     if (threadIdx.x == 0 && visits > 0) {   // (a sector that hit the limit stays unfinished: svd_kernel reports it)
       atomicMin(&done_at[e], visits * R - 1);
