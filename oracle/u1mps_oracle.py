@@ -24,7 +24,7 @@ Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): P1 exact state vector (M<=
 invariants, P3 unit norm, P4 canonical-form identities, P5 Eckart-Young reconstruction, P6 brute
 force dense (non-symmetric) update Eq.11-14, P7 identity/swap gates, P8 closed forms (single
 particle walk, permanents, Hong-Ou-Mandel), P9 free-fermion <n_k>, P10 readout formula vs full
-environments.  Every function below is reached by at least one of them; nothing is
+environments, P11 tie order at the cut, P12 two-point <n_j n_k> vs the state vector.  Every function below is reached by at least one of them; nothing is
 "parity unpinned".
 """
 from __future__ import annotations
@@ -286,6 +286,55 @@ class U1MPS:
             if cl in envL[s] and cr in Rr:
                 a = A(s, cl, cr)
                 val += (cl - cr) * float(np.real(np.trace(a.conj().T @ envL[s][cl] @ a @ Rr[cr])))
+        return val / norm
+
+    def expect_nn_full(self, j: int, k: int) -> float:
+        """<psi|n_j n_k|psi>/<psi|psi>, j <= k, with explicitly contracted environments (pin P12).
+
+        Same contraction as expect_n_full (state of Eq.15): the occupation of a site is the charge
+        difference of its two bonds, so n_j inserts the weight (c_l - c_r) into the transfer step of site j.
+        """
+        if j > k:
+            j, k = k, j
+
+        def A(site, cl, cr):
+            return self.gam[site][(cl, cr)] * self.lam[site + 1][cr][None, :]
+        E = {self.N: np.ones((1, 1), dtype=np.complex128)}
+        F = None                                   # left environment with n_j inserted, from bond j+1 on
+        for site in range(k):
+            En: Dict[int, np.ndarray] = {}
+            Fn: Dict[int, np.ndarray] = {}
+            for (cl, cr) in self.gam[site]:
+                a = A(site, cl, cr)
+                if cl in E:
+                    En[cr] = En.get(cr, 0) + a.conj().T @ E[cl] @ a
+                    if site == j:
+                        Fn[cr] = Fn.get(cr, 0) + (cl - cr) * (a.conj().T @ E[cl] @ a)
+                if F is not None and cl in F:
+                    Fn[cr] = Fn.get(cr, 0) + a.conj().T @ F[cl] @ a
+            E = En
+            if site >= j:
+                F = Fn
+        Rr = {0: np.ones((1, 1), dtype=np.complex128)}
+        for site in range(self.M - 1, k, -1):
+            Rn: Dict[int, np.ndarray] = {}
+            for (cl, cr) in self.gam[site]:
+                if cr in Rr:
+                    a = A(site, cl, cr)
+                    Rn[cl] = Rn.get(cl, 0) + a @ Rr[cr] @ a.conj().T
+            Rr = Rn
+        val, norm = 0.0, 0.0
+        for (cl, cr) in self.gam[k]:
+            if cr not in Rr:
+                continue
+            a = A(k, cl, cr)
+            if cl in E:
+                t = float(np.real(np.trace(a.conj().T @ E[cl] @ a @ Rr[cr])))
+                norm += t
+                if j == k:
+                    val += (cl - cr) ** 2 * t
+            if j < k and F is not None and cl in F:
+                val += (cl - cr) * float(np.real(np.trace(a.conj().T @ F[cl] @ a @ Rr[cr])))
         return val / norm
 
     def to_dense(self):

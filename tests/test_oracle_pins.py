@@ -436,3 +436,27 @@ def test_P11_tie_order_and_keep_at_least_one():
         assert {c: k for c, k in rec.keep.items() if k > 0} == want, (chi, rec.keep, want)
     sig = sorted((float(x), c) for c, v in rec.sigma.items() for x in v if x > 1e-12)
     assert any(abs(x - y) == 0.0 and c1 != c2 for (x, c1), (y, c2) in zip(sig[:-1], sig[1:]))   # ties across sectors exist
+
+
+# ------------------------------------------------------------------ P12: two-point function with explicit environments
+def test_P12_two_point_function_matches_state_vector():
+    """<n_j n_k> from the environment contraction against the plain state vector (digit sums over the d^M amplitudes),
+    on an untruncated state and on a truncated one (compared with the state vector of the TRUNCATED MPS, rebuilt from
+    its amplitudes: the contraction is exact for whatever state the MPS holds)."""
+    rng = np.random.default_rng(77)
+    d, M, N = 3, 6, 5
+    occ = [2, 0, 1, 1, 0, 1]
+    gates = brick_gates(rng, M, d, 3, lambda r: inputs.random_u1_gate(r, d))
+    for chi in (d ** 3, 4):
+        st = U1MPS.product_state(M, d, N, chi, occ)
+        for s, U in gates:
+            st.apply_gate(s, U, chi=chi, cutoff=1e-12)
+        vec = st.amplitudes()
+        p = np.abs(vec) ** 2
+        p = p / p.sum()
+        digits = np.array(list(itertools.product(range(d), repeat=M)))      # site 0 = most significant digit (S23)
+        for j in range(M):
+            for k in range(j, M):
+                ref = float(np.sum(p * digits[:, j] * digits[:, k]))
+                assert abs(st.expect_nn_full(j, k) - ref) < 1e-12, (chi, j, k)
+        assert abs(sum(st.expect_nn_full(j, k) * (1 if j == k else 2) for j in range(M) for k in range(j, M)) - N * N) < 1e-10
