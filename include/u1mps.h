@@ -115,6 +115,11 @@ int u1mps_bond_entropy_all(u1mps_t* h, double* out_host /*[M+1]*/);
  * buffers); U1MPS_ENOMEM if it is too small.  out_host: [M].  Both [sync]. */
 int u1mps_expect_n_full_bytes(u1mps_t* h, size_t* bytes_host);
 int u1mps_expect_n_full(u1mps_t* h, double* out_host, void* scratch_dev, size_t scratch_bytes);
+/* Two-point function <psi|n_j n_k|psi> / <psi|psi> (any order of j, k; j == k gives <n_j^2>), the same environment
+ * sweeps with the occupation c_l - c_r inserted into the transfer step of site j (state of Eq.15).  Device
+ * scratch of at least u1mps_expect_nn_full_bytes (six environment-sized and two Gamma-sized buffers).  Both [sync]. */
+int u1mps_expect_nn_full_bytes(u1mps_t* h, size_t* bytes_host);
+int u1mps_expect_nn_full(u1mps_t* h, int site_j, int site_k, double* out_host, void* scratch_dev, size_t scratch_bytes);
 /* Sector table of a bond: writes up to cap (charge, count) pairs, ascending charge; *n_sectors = how many exist. */
 int u1mps_bond_info(u1mps_t* h, int bond, int32_t* n_sectors, int32_t* charges, int32_t* counts, int cap);
 int u1mps_bond_dims(u1mps_t* h, int32_t* dims_host /*[M+1]*/);

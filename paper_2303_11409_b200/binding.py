@@ -23,6 +23,7 @@ EXPORTS = [
     "u1mps_import_site", "u1mps_set_log_norm", "u1mps_staged_info", "u1mps_export_staged_theta",
     "u1mps_export_staged_svd", "u1mps_launch_count", "u1mps_profile_enable", "u1mps_profile_read",
     "u1mps_stage_name", "u1mps_svd_trace", "u1mps_clear_status", "u1mps_expect_n_full_bytes", "u1mps_expect_n_full",
+    "u1mps_expect_nn_full_bytes", "u1mps_expect_nn_full",
 ]
 NSTAGE = 8
 
@@ -86,6 +87,8 @@ def load_library() -> C.CDLL:
     lib.u1mps_clear_status.argtypes = [vp]
     lib.u1mps_expect_n_full_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     lib.u1mps_expect_n_full.argtypes = [vp, dp, vp, C.c_size_t]
+    lib.u1mps_expect_nn_full_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+    lib.u1mps_expect_nn_full.argtypes = [vp, C.c_int, C.c_int, dp, vp, C.c_size_t]
     lib.u1mps_stage_name.restype = C.c_char_p
     lib.u1mps_stage_name.argtypes = [C.c_int]
     for name in EXPORTS:
@@ -219,6 +222,16 @@ class U1MPS:
         out = np.zeros(self.M)
         self._ck(self.lib.u1mps_expect_n_full(self.h, _ptr(out, C.POINTER(C.c_double)), C.c_void_p(scratch.data_ptr()), nbytes.value))
         return out
+
+    def expect_nn_full(self, j: int, k: int) -> float:
+        """<psi|n_j n_k|psi> / <psi|psi> with explicit environments."""
+        import torch
+        nbytes = C.c_size_t()
+        self._ck(self.lib.u1mps_expect_nn_full_bytes(self.h, C.byref(nbytes)))
+        scratch = torch.empty(max(nbytes.value, 256), dtype=torch.uint8, device="cuda")
+        v = C.c_double()
+        self._ck(self.lib.u1mps_expect_nn_full(self.h, j, k, C.byref(v), C.c_void_p(scratch.data_ptr()), nbytes.value))
+        return v.value
 
     def bond_entropy(self, bond: int) -> float:
         v = C.c_double()

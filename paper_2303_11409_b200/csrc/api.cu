@@ -473,6 +473,32 @@ int u1mps_expect_n_full(u1mps_t* h, double* out, void* scratch_dev, size_t scrat
   return U1MPS_OK;
 }
 
+int u1mps_expect_nn_full_bytes(u1mps_t* h, size_t* bytes) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
+  if (!h || !bytes) return U1MPS_EINVAL;
+  if (h->stage != ST_NONE) return U1MPS_ESTAGED;
+  std::vector<long long> gamoff, gused;
+  int r = env_tables(h, gamoff, gused);
+  if (r) return r;
+  *bytes = u1_env_nn_scratch_bytes(h->M, h->NC, h->d, h->h_nb, gused);
+  return U1MPS_OK;
+}
+
+int u1mps_expect_nn_full(u1mps_t* h, int site_j, int site_k, double* out, void* scratch_dev, size_t scratch_bytes) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
+  if (!h || !out || !scratch_dev || ((uintptr_t)scratch_dev & 255) || site_j < 0 || site_k < 0 || site_j >= h->M || site_k >= h->M)
+    return U1MPS_EINVAL;
+  if (h->stage != ST_NONE) return U1MPS_ESTAGED;
+  std::vector<long long> gamoff, gused;
+  int r = env_tables(h, gamoff, gused);
+  if (r) return r;
+  if (scratch_bytes < u1_env_nn_scratch_bytes(h->M, h->NC, h->d, h->h_nb, gused)) return U1MPS_ENOMEM;
+  CK(u1_env_expect_nn(h->S, h->h_nb, gamoff, gused, std::min(site_j, site_k), std::max(site_j, site_k), scratch_dev, h->dout, h->L));
+  CK(cudaMemcpyAsync(out, h->dout, 8, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return U1MPS_OK;
+}
+
 int u1mps_bond_entropy_all(u1mps_t* h, double* out) {
   if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out) return U1MPS_EINVAL;

@@ -131,5 +131,8 @@ void u1_launch_product_state(const DevState& S, const int* occ_dev, const Launch
 void u1_launch_gamoff(const DevState& S, int site, const LaunchCfg& L);
 cudaError_t u1_svd_configure(int* grid, int* smem_bytes, int sms);
 size_t u1_env_scratch_bytes(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused);
+size_t u1_env_nn_scratch_bytes(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused);
+cudaError_t u1_env_expect_nn(const DevState& S, const std::vector<int>& nb, const std::vector<long long>& gamoff,
+                             const std::vector<long long>& gused, int j, int k, void* scratch, double* out_dev, const LaunchCfg& L);
 cudaError_t u1_env_expect_n(const DevState& S, const std::vector<int>& nb, const std::vector<long long>& gamoff,
                             const std::vector<long long>& gused, void* scratch, double* out_dev, const LaunchCfg& L);

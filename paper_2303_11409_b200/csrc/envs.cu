@@ -24,6 +24,7 @@ struct EnvDesc {
   const cplx* B[EV_MAXTERM];     // ... right operand (k x n, or n x k if opB)
   const double* ks[EV_MAXTERM];  // ... optional scale over the inner index (nullptr: none)
   int k[EV_MAXTERM];
+  double w[EV_MAXTERM];          // ... weight of the term (the occupation, for an inserted n)
   cplx* C;                       // m x n row-major
   const double* rs;              // optional output row / column scales
   const double* cs;
@@ -52,6 +53,7 @@ __global__ void __launch_bounds__(EV_THREADS) env_gemm_kernel(const EnvDesc* __r
       const cplx* B = D.B[t];
       const double* ks = D.ks[t];
       const int K = D.k[t];
+      const double wt = D.w[t];
       for (int k0 = 0; k0 < K; k0 += EV_KC) {
         cplx ra[4], rb[4];
         // A chunk: 32 (a) x 16 (kk)
@@ -62,7 +64,8 @@ __global__ void __launch_bounds__(EV_THREADS) env_gemm_kernel(const EnvDesc* __r
             const int a = (tid >> 4) + 8 * x;
             cplx v = make_double2(0.0, 0.0);
             if (a0 + a < m && k0 + kk < K) v = A[(long long)(a0 + a) * K + k0 + kk];
-            if (ks && k0 + kk < K) { const double sc = ks[k0 + kk]; v.x *= sc; v.y *= sc; }
+            const double sc = (ks && k0 + kk < K) ? wt * ks[k0 + kk] : wt;
+            v.x *= sc; v.y *= sc;
             ra[x] = v;
           }
         } else {        // stored K x m, conjugated: a fastest
@@ -72,7 +75,8 @@ __global__ void __launch_bounds__(EV_THREADS) env_gemm_kernel(const EnvDesc* __r
             const int kk = (tid >> 5) + 4 * x;
             cplx v = make_double2(0.0, 0.0);
             if (a0 + a < m && k0 + kk < K) { v = A[(long long)(k0 + kk) * m + a0 + a]; v.y = -v.y; }
-            if (ks && k0 + kk < K) { const double sc = ks[k0 + kk]; v.x *= sc; v.y *= sc; }
+            const double sc = (ks && k0 + kk < K) ? wt * ks[k0 + kk] : wt;
+            v.x *= sc; v.y *= sc;
             ra[x] = v;
           }
         }
@@ -265,7 +269,7 @@ cudaError_t u1_env_expect_n(const DevState& S, const std::vector<int>& nb, const
     ++la.nd;
   };
   EnvDesc Z;
-  for (int t = 0; t < EV_MAXTERM; ++t) { Z.A[t] = nullptr; Z.B[t] = nullptr; Z.ks[t] = nullptr; Z.k[t] = 0; }
+  for (int t = 0; t < EV_MAXTERM; ++t) { Z.A[t] = nullptr; Z.B[t] = nullptr; Z.ks[t] = nullptr; Z.k[t] = 0; Z.w[t] = 1.0; }
   Z.C = nullptr; Z.rs = nullptr; Z.cs = nullptr; Z.alpha = 1.0; Z.m = Z.n = Z.nterm = Z.opA = Z.opB = 0;
   for (int s = 0; s < M; ++s) {
     const cplx* G = S.gam + (size_t)s * S.gcap;
@@ -352,6 +356,191 @@ cudaError_t u1_env_expect_n(const DevState& S, const std::vector<int>& nb, const
     run(LA[(size_t)s * 5 + 4]);
   }
   env_finish_kernel<<<1, 256, 0, L.stream>>>(out_dev, M, Eptr(M, 0));
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Two-point function <psi|n_j n_k|psi> / <psi|psi>, j <= k: the same sweeps with the weight
+// (c_l - c_r) inserted into the transfer step of site j; F is the left environment that carries the insertion.
+//   F_{j+1}[cr] = sum_cl (cl - cr) A^H E_j[cl] A,   F_{s+1}[cr] = sum_cl A^H F_s[cl] A  (s > j)
+//   value = sum (cl - cr) tr(A^H F_k[cl] A R_{k+1}[cr])      (j < k;  (cl - cr)^2 and E_k for j == k)
+//   norm  = sum tr(A^H E_k[cl] A R_{k+1}[cr])
+__global__ void env_ratio_kernel(double* out, const double* val, const double* norm) { *out = *val / *norm; }
+
+namespace {
+struct NNLayout { long long maxE = 0, maxG = 0; size_t ndesc = 0, npref = 0, o_desc = 0, o_pref = 0, o_E = 0, o_F = 0, o_R = 0, o_T = 0, o_S = 0, o_misc = 0, total = 0; };
+NNLayout nn_layout(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused) {
+  NNLayout Y;
+  size_t per_site = 0;
+  for (int k = 0; k <= M; ++k) {
+    long long run = 0; size_t nsec = 0;
+    for (int c = 0; c < NC; ++c) { const long long n = nb[(size_t)k * NC + c]; run += n * n; nsec += n > 0; }
+    Y.maxE = std::max(Y.maxE, run);
+    per_site = std::max(per_site, nsec);
+  }
+  size_t maxblk = 0;
+  for (int s = 0; s < M; ++s) {
+    Y.maxG = std::max(Y.maxG, gused[s]);
+    size_t nblk = 0;
+    for (int cl = 0; cl < NC; ++cl) for (int i = 0; i < d && cl - i >= 0; ++i)
+      if (nb[(size_t)s * NC + cl] && nb[(size_t)(s + 1) * NC + cl - i]) ++nblk;
+    maxblk = std::max(maxblk, nblk);
+  }
+  Y.ndesc = (size_t)(M + 2) * (2 * maxblk + 3 * per_site + 2);   // generous: at most 2 block launches + 3 sector launches per site
+  Y.npref = Y.ndesc + (size_t)(M + 2) * 6;
+  size_t o = 0;
+  Y.o_desc = o; o = al256(o + Y.ndesc * sizeof(EnvDesc));
+  Y.o_pref = o; o = al256(o + Y.npref * sizeof(int));
+  Y.o_E = o;    o = al256(o + (size_t)2 * Y.maxE * sizeof(cplx));
+  Y.o_F = o;    o = al256(o + (size_t)2 * Y.maxE * sizeof(cplx));
+  Y.o_R = o;    o = al256(o + (size_t)2 * Y.maxE * sizeof(cplx));
+  Y.o_T = o;    o = al256(o + (size_t)Y.maxG * sizeof(cplx));
+  Y.o_S = o;    o = al256(o + (size_t)Y.maxG * sizeof(cplx));
+  Y.o_misc = o; o = al256(o + (EV_DOT_SLICES + 8) * sizeof(double));
+  Y.total = o;
+  return Y;
+}
+}  // namespace
+
+size_t u1_env_nn_scratch_bytes(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused) {
+  return nn_layout(M, NC, d, nb, gused).total;
+}
+
+cudaError_t u1_env_expect_nn(const DevState& S, const std::vector<int>& nb, const std::vector<long long>& gamoff,
+                             const std::vector<long long>& gused, int j, int k, void* scratch, double* out_dev, const LaunchCfg& L) {
+  const int M = S.M, NC = S.NC, d = S.d;
+  const NNLayout Y = nn_layout(M, NC, d, nb, gused);
+  char* base = (char*)scratch;
+  EnvDesc* d_desc = (EnvDesc*)(base + Y.o_desc);
+  int* d_pref = (int*)(base + Y.o_pref);
+  cplx* Ebuf = (cplx*)(base + Y.o_E);
+  cplx* Fbuf = (cplx*)(base + Y.o_F);
+  cplx* Rbuf = (cplx*)(base + Y.o_R);
+  cplx* Tbuf = (cplx*)(base + Y.o_T);
+  cplx* Sbuf = (cplx*)(base + Y.o_S);
+  double* part = (double*)(base + Y.o_misc);
+  int* count = (int*)(part + EV_DOT_SLICES);
+  double* scal = part + EV_DOT_SLICES + 2;   // [0] value, [1] norm
+  std::vector<int> ob((size_t)(M + 1) * NC);
+  std::vector<long long> eoff((size_t)(M + 1) * NC);
+  for (int b = 0; b <= M; ++b) {
+    int run = 0; long long er = 0;
+    for (int c = 0; c < NC; ++c) { ob[(size_t)b * NC + c] = run; eoff[(size_t)b * NC + c] = er; const long long n = nb[(size_t)b * NC + c]; run += (int)n; er += n * n; }
+  }
+  auto nK = [&](int b, int c) { return nb[(size_t)b * NC + c]; };
+  auto envp = [&](cplx* buf, int b, int c) { return buf + (size_t)(b & 1) * Y.maxE + eoff[(size_t)b * NC + c]; };
+  auto lamp = [&](int b, int c) { return S.lam + (size_t)b * S.chi + ob[(size_t)b * NC + c]; };
+  auto goff = [&](int s, int cl, int i) { return gamoff[((size_t)s * NC + cl) * d + i]; };
+  struct Launch { size_t d0, p0; int nd, tiles; };
+  std::vector<EnvDesc> descs;
+  std::vector<int> prefs;
+  std::vector<Launch> order;
+  EnvDesc Z;
+  for (int t = 0; t < EV_MAXTERM; ++t) { Z.A[t] = nullptr; Z.B[t] = nullptr; Z.ks[t] = nullptr; Z.k[t] = 0; Z.w[t] = 1.0; }
+  Z.C = nullptr; Z.rs = nullptr; Z.cs = nullptr; Z.alpha = 1.0; Z.m = Z.n = Z.nterm = Z.opA = Z.opB = 0;
+  Launch cur;
+  auto begin = [&]() { cur.d0 = descs.size(); cur.p0 = prefs.size(); cur.nd = 0; cur.tiles = 0; prefs.push_back(0); };
+  auto push = [&](const EnvDesc& D) { descs.push_back(D); cur.tiles += u1_ceil_div(D.m, U1_TILE) * u1_ceil_div(D.n, U1_TILE); prefs.push_back(cur.tiles); ++cur.nd; };
+  auto end = [&]() { order.push_back(cur); };
+  // dst_f = alpha(i) env[cl] Gamma_f for the blocks of site s (alpha == 0: skipped)
+  auto mkT = [&](int s, cplx* env, cplx* dst, int power) {
+    begin();
+    const cplx* G = S.gam + (size_t)s * S.gcap;
+    for (int cl = 0; cl < NC; ++cl) for (int i = 0; i < d && cl - i >= 0; ++i) {
+      const int nl = nK(s, cl), nr = nK(s + 1, cl - i);
+      if (!nl || !nr) continue;
+      const double al = power == 0 ? 1.0 : power == 1 ? (double)i : (double)i * i;
+      if (al == 0.0) continue;
+      EnvDesc D = Z; D.m = nl; D.n = nr; D.nterm = 1; D.A[0] = envp(env, s, cl); D.B[0] = G + goff(s, cl, i); D.k[0] = nl; D.C = dst + goff(s, cl, i); D.alpha = al;
+      push(D);
+    }
+    end();
+  };
+  // env'[cr] = lam (sum_i w_i Gamma_f^H src_f) lam for the sectors of bond s+1 (weighted: w_i = i)
+  auto mkL2 = [&](int s, const cplx* src, cplx* env, bool weighted) {
+    begin();
+    const cplx* G = S.gam + (size_t)s * S.gcap;
+    for (int cr = 0; cr < NC; ++cr) {
+      const int nr = nK(s + 1, cr);
+      if (!nr) continue;
+      EnvDesc D = Z; D.m = nr; D.n = nr; D.opA = 1; D.C = envp(env, s + 1, cr); D.rs = lamp(s + 1, cr); D.cs = lamp(s + 1, cr);
+      for (int i = weighted ? 1 : 0; i < d && cr + i < NC; ++i) {
+        const int nl = nK(s, cr + i);
+        if (!nl) continue;
+        D.A[D.nterm] = G + goff(s, cr + i, i); D.B[D.nterm] = src + goff(s, cr + i, i); D.k[D.nterm] = nl; D.w[D.nterm] = weighted ? (double)i : 1.0; ++D.nterm;
+      }
+      push(D);
+    }
+    end();
+  };
+  auto mkR1 = [&](int s) {   // S_f = Gamma_f lam R_{s+1}[cr] lam
+    begin();
+    const cplx* G = S.gam + (size_t)s * S.gcap;
+    for (int cl = 0; cl < NC; ++cl) for (int i = 0; i < d && cl - i >= 0; ++i) {
+      const int nl = nK(s, cl), nr = nK(s + 1, cl - i);
+      if (!nl || !nr) continue;
+      EnvDesc D = Z; D.m = nl; D.n = nr; D.nterm = 1; D.A[0] = G + goff(s, cl, i); D.ks[0] = lamp(s + 1, cl - i); D.B[0] = envp(Rbuf, s + 1, cl - i);
+      D.k[0] = nr; D.cs = lamp(s + 1, cl - i); D.C = Sbuf + goff(s, cl, i);
+      push(D);
+    }
+    end();
+  };
+  auto mkR2 = [&](int s) {   // R_s[cl] = sum_i S_f Gamma_f^H
+    begin();
+    const cplx* G = S.gam + (size_t)s * S.gcap;
+    for (int cl = 0; cl < NC; ++cl) {
+      const int nl = nK(s, cl);
+      if (!nl) continue;
+      EnvDesc D = Z; D.m = nl; D.n = nl; D.opB = 1; D.C = envp(Rbuf, s, cl);
+      for (int i = 0; i < d && cl - i >= 0; ++i) {
+        const int nr = nK(s + 1, cl - i);
+        if (!nr) continue;
+        D.A[D.nterm] = Sbuf + goff(s, cl, i); D.B[D.nterm] = G + goff(s, cl, i); D.k[D.nterm] = nr; ++D.nterm;
+      }
+      push(D);
+    }
+    end();
+  };
+  // launch order; entries of `order` are consumed in this order below, interleaved with the memsets and dots
+  for (int s = 0; s < k; ++s) {
+    mkT(s, Ebuf, Tbuf, 0); mkL2(s, Tbuf, Ebuf, false);
+    if (s == j) mkL2(s, Tbuf, Fbuf, true);
+    else if (s > j) { mkT(s, Fbuf, Sbuf, 0); mkL2(s, Sbuf, Fbuf, false); }
+  }
+  for (int s = M - 1; s > k; --s) { mkR1(s); mkR2(s); }
+  mkR1(k);
+  mkT(k, Ebuf, Tbuf, 0);                              // norm
+  if (j < k) mkT(k, Fbuf, Tbuf, 1); else mkT(k, Ebuf, Tbuf, 2);   // value
+  if (descs.size() > Y.ndesc || prefs.size() > Y.npref) return cudaErrorInvalidValue;
+  cudaError_t err;
+  if ((err = cudaMemcpyAsync(d_desc, descs.data(), descs.size() * sizeof(EnvDesc), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemcpyAsync(d_pref, prefs.data(), prefs.size() * sizeof(int), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemsetAsync(Ebuf, 0, (size_t)2 * Y.maxE * sizeof(cplx), L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemsetAsync(Fbuf, 0, (size_t)2 * Y.maxE * sizeof(cplx), L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemsetAsync(Rbuf, 0, (size_t)2 * Y.maxE * sizeof(cplx), L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemsetAsync(part, 0, (EV_DOT_SLICES + 8) * sizeof(double), L.stream)) != cudaSuccess) return err;
+  const cplx one = make_double2(1.0, 0.0);
+  if ((err = cudaMemcpyAsync(envp(Ebuf, 0, S.N), &one, sizeof(cplx), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemcpyAsync(envp(Rbuf, M, 0), &one, sizeof(cplx), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  auto run = [&](const Launch& la) {
+    if (la.tiles == 0) return;
+    L.prof->begin(U1_ST_READOUT, L.stream);
+    env_gemm_kernel<<<std::min(la.tiles, L.sms * 8), EV_THREADS, 0, L.stream>>>(d_desc + la.d0, d_pref + la.p0, la.nd);
+    L.prof->end(L.stream);
+    ++*L.launches;
+  };
+  const size_t n_final = 3;   // R1(k), T(norm), T(value)
+  for (size_t q = 0; q + n_final < order.size(); ++q) run(order[q]);
+  const size_t q0 = order.size() - n_final;
+  run(order[q0]);                                       // S_f at site k
+  for (int pass = 0; pass < 2; ++pass) {                // norm, then value
+    if ((err = cudaMemsetAsync(Tbuf, 0, (size_t)gused[k] * sizeof(cplx), L.stream)) != cudaSuccess) return err;
+    run(order[q0 + 1 + pass]);
+    env_dot_kernel<<<EV_DOT_SLICES, EV_DOT_THREADS, 0, L.stream>>>(Tbuf, Sbuf, gused[k], part, count, scal + (pass == 0 ? 1 : 0));
+    ++*L.launches;
+  }
+  env_ratio_kernel<<<1, 1, 0, L.stream>>>(out_dev, scal, scal + 1);
   ++*L.launches;
   return cudaGetLastError();
 }

@@ -196,6 +196,22 @@ def test_expect_n_full_on_truncated_states(idx, M, N, chi, cols):
     assert np.allclose(fresh.expect_n_full(), w.occ, atol=1e-15)
 
 
+@pytest.mark.parametrize("idx,M,N,chi,cols", [(2, 12, 6, 8, 12), (4, 8, 4, 6, 8), (5, 10, 5, 6, 10)])
+def test_expect_nn_full_on_truncated_states(idx, M, N, chi, cols):
+    """u1mps_expect_nn_full = <psi|n_j n_k|psi>/<psi|psi> against the oracle's expect_nn_full (pinned by P12 against the
+    state vector) for every pair j <= k of truncated reduced chains: 1e-9 each, and sum_jk = N^2."""
+    w = inputs.small_variant(inputs.WORKLOADS[idx], M=M, N=N, chi=chi, columns=cols)
+    ora, gpu = run_both(w)
+    tot = 0.0
+    for j in range(w.M):
+        for k in range(j, w.M):
+            got, want = gpu.expect_nn_full(j, k), ora.expect_nn_full(j, k)
+            assert abs(got - want) <= 1e-9, (j, k, got, want)
+            tot += got * (1 if j == k else 2)
+    assert abs(tot - w.N ** 2) <= 1e-8
+    assert gpu.expect_nn_full(3, 1) == gpu.expect_nn_full(1, 3)
+
+
 # ------------------------------------------------------------------ the tie order at the cut (reading S8)
 def test_exact_tie_at_the_cut_and_keep_at_least_one():
     """An exact tie across two sectors at the cut: |10> under a gate with equal amplitudes to stay and to hop gives
