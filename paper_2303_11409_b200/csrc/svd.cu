@@ -44,9 +44,13 @@ static_assert(U1_MAXSWEEP == 30, "keep U1MPS_MAXSWEEP of include/u1mps.h in step
 #ifndef SV_TOLFAC
 #define SV_TOLFAC 8.0                // stopping threshold tol = SV_TOLFAC eps sqrt(m) on |h_pq| / sqrt(h_pp h_qq)
 #endif
+#ifndef SV_INNER_MAX
 #define SV_INNER_MAX 2               // inner EVD sweeps per item (the outer iteration finishes the job; measured best of 1..4)
+#endif
 #define SV_LASTPASS 1e-18            // (relative off-diagonal)^2 below which a rotation needs no verification sweep
+#ifndef SV_QUAD
 #define SV_QUAD 1e-4                 // no second inner sweep after one whose largest relative off-diagonal^2 was below this (measured best of 1e-14 .. 3e-1)
+#endif
 #define SV_GROUP 128                 // threads per pair item (= one CTA: SV_NGROUP == 1; several groups per CTA were tried and dropped)
 #define SV_NGROUP (U1_SVD_THREADS / SV_GROUP)
 #ifndef SV_CTAS
