@@ -42,11 +42,12 @@ enum {
   U1MPS_ENOMEM = -4,  /* arena too small for this call */
   U1MPS_ECUDA = -5,   /* CUDA error, or no CUDA device.  Sticky: once a CUDA runtime call of a handle has failed, every
                          later call on that handle returns U1MPS_ECUDA */
-  U1MPS_ENOCONV = -6  /* Jacobi SVD hit the sweep limit on some sector.  Detected on the device, so it is reported by the
+  U1MPS_ENOCONV = -6, /* Jacobi SVD hit the sweep limit on some sector.  Detected on the device, so it is reported by the
                          [sync] calls that read the device status (log_norm, norm2, last_stats, staged_info,
                          export_staged_svd).  Sticky, like U1MPS_ENOMEM raised by a launch whose plan did not fit the arena:
                          it stays set until u1mps_clear_status or u1mps_set_product_state, so that a failure in any gate
                          since the last check is never lost */
+  U1MPS_ETOOBIG = -7  /* a size beyond the fixed maximum of a no-allocation entry point (u1mps_expect_n_all_static) */
 };
 
 const char* u1mps_strerror(int code);
@@ -107,6 +108,22 @@ int u1mps_expect_n(u1mps_t* h, int site, double* out_host);        /* canonical-
 int u1mps_expect_n_all(u1mps_t* h, double* out_host /*[M]*/);      /* all sites, one launch */
 int u1mps_bond_entropy(u1mps_t* h, int bond, double* out_host);    /* -sum lambda^2 ln lambda^2 (natural log, S23) */
 int u1mps_bond_entropy_all(u1mps_t* h, double* out_host /*[M+1]*/);
+/* u1mps_expect_n_all for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): the same kernel and the same canonical-form <n_s> of all sites (Eq.10, Eq.15),
+ * with the kernel's scratch (the partial sums of the slices a site is cut into and one completion counter per site) in
+ * a static device array of the library instead of the arena: 69 632 bytes on every GPU that loads the library, held
+ * until the process exits.  The call makes no cudaMalloc / cudaFree and no allocating library call: it enqueues one
+ * memset (the counters it uses must start at zero; the array keeps the previous call's contents) and one kernel on the
+ * handle's stream and returns WITHOUT synchronising.  [async]
+ *   out_dev: DEVICE double[M], 8-byte aligned, owned by the caller, on the device the handle lives on (which must be
+ *            the current device); valid once the handle's stream has reached this point.  A host pointer -> U1MPS_EINVAL.
+ *   M > U1MPS_STATIC_SITES_MAX -> U1MPS_ETOOBIG (nothing is enqueued); U1MPS_ESTAGED while a gate is staged.
+ * Every handle and every call on a device shares the one array: calls that overlap on the GPU (handles on different
+ * streams without an ordering between them) race on it and return garbage - serialise them.  Calls on one stream are
+ * ordered and safe.  The sums are added in the same fixed order as in u1mps_expect_n_all (bit-identical results as long
+ * as M <= U1MPS_STATIC_SITES_MAX, which keeps the slice count the same). */
+#define U1MPS_STATIC_SITES_MAX 1024
+int u1mps_expect_n_all_static(u1mps_t* h, double* out_dev /*[M]*/);
 /* Full-environment <psi|n_k|psi> / <psi|psi> of all sites (state of Eq.15): left and
  * right environments contracted explicitly, exact for whatever Gamma, lambda the handle holds - unlike the
  * canonical-form u1mps_expect_n, which is exact only while nothing has been truncated (Eq.10).  The caller

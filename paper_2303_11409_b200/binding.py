@@ -23,11 +23,13 @@ EXPORTS = [
     "u1mps_import_site", "u1mps_set_log_norm", "u1mps_staged_info", "u1mps_export_staged_theta",
     "u1mps_export_staged_svd", "u1mps_launch_count", "u1mps_profile_enable", "u1mps_profile_read",
     "u1mps_stage_name", "u1mps_svd_trace", "u1mps_clear_status", "u1mps_expect_n_full_bytes", "u1mps_expect_n_full",
-    "u1mps_expect_nn_full_bytes", "u1mps_expect_nn_full",
+    "u1mps_expect_nn_full_bytes", "u1mps_expect_nn_full", "u1mps_expect_n_all_static",
 ]
 NSTAGE = 8
 
 ENOCONV = -6
+ETOOBIG = -7
+STATIC_SITES_MAX = 1024   # U1MPS_STATIC_SITES_MAX
 
 
 class U1MPSError(RuntimeError):
@@ -89,6 +91,7 @@ def load_library() -> C.CDLL:
     lib.u1mps_expect_n_full.argtypes = [vp, dp, vp, C.c_size_t]
     lib.u1mps_expect_nn_full_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     lib.u1mps_expect_nn_full.argtypes = [vp, C.c_int, C.c_int, dp, vp, C.c_size_t]
+    lib.u1mps_expect_n_all_static.argtypes = [vp, vp]
     lib.u1mps_stage_name.restype = C.c_char_p
     lib.u1mps_stage_name.argtypes = [C.c_int]
     for name in EXPORTS:
@@ -212,6 +215,14 @@ class U1MPS:
         out = np.zeros(self.M)
         self._ck(self.lib.u1mps_expect_n_all(self.h, _ptr(out, C.POINTER(C.c_double))))
         return out
+
+    def expect_n_all_static(self, out_dev) -> None:
+        """u1mps_expect_n_all on the library's static scratch: no allocation, no synchronisation.  out_dev: a CUDA
+        float64 tensor of M elements that the caller owns; it is valid once the handle's stream has got there."""
+        if not (out_dev.is_cuda and out_dev.dtype.is_floating_point and out_dev.element_size() == 8
+                and out_dev.is_contiguous() and out_dev.numel() >= self.M):
+            raise U1MPSError(-1, "out_dev must be a contiguous CUDA float64 tensor of at least M elements")
+        self._ck(self.lib.u1mps_expect_n_all_static(self.h, C.c_void_p(out_dev.data_ptr())))
 
     def expect_n_full(self) -> np.ndarray:
         """<psi|n_k|psi> / <psi|psi> with explicit environments (exact also after truncation); scratch from torch."""

@@ -213,6 +213,7 @@ const char* u1mps_strerror(int code) {
     case U1MPS_ENOMEM: return "arena too small";
     case U1MPS_ECUDA: return "CUDA error or no CUDA device";
     case U1MPS_ENOCONV: return "Jacobi SVD did not converge within the sweep limit";
+    case U1MPS_ETOOBIG: return "size beyond the fixed maximum of a no-allocation entry point";
     default: return "unknown error";
   }
 }
@@ -430,6 +431,21 @@ int u1mps_expect_n(u1mps_t* h, int site, double* out) {
   CK(cudaGetLastError());
   CK(cudaMemcpyAsync(out, h->dout + site, 8, cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
+  return U1MPS_OK;
+}
+
+// a6 for callers that must not allocate: scratch in a static device array of readout.cu, result left on the device, no
+// host synchronisation; nothing here or below calls cudaMalloc / cudaFree or an allocating library routine.
+static_assert(U1_RD_STATIC_SITES == U1MPS_STATIC_SITES_MAX, "keep include/u1mps.h in step");
+int u1mps_expect_n_all_static(u1mps_t* h, double* out_dev) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
+  if (!h || !out_dev) return U1MPS_EINVAL;
+  if (h->stage != ST_NONE) return U1MPS_ESTAGED;
+  if (h->M > U1MPS_STATIC_SITES_MAX) return U1MPS_ETOOBIG;
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, out_dev) != cudaSuccess) { cudaGetLastError(); return U1MPS_EINVAL; }
+  if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) return U1MPS_EINVAL;   // a host pointer
+  CK(u1_launch_expect_n_static(h->S, h->M, out_dev, h->L));
   return U1MPS_OK;
 }
 

@@ -12,6 +12,7 @@ typedef double2 cplx;  // complex128, interleaved (x = re, y = im), 16-byte alig
 #define U1_ERR_WORKSPACE 1 // device error flag: plan does not fit the workspace
 #define U1_ERR_SCHED 2     // device error flag: an a3 work-queue dependency did not resolve (internal error)
 #define U1_RD_SLICES 1024   // a6: at most this many CTAs share one site
+#define U1_RD_STATIC_SITES 1024   // a6 on static scratch: longest chain (= U1MPS_STATIC_SITES_MAX of include/u1mps.h)
 #define U1_SCHED 264       // entries of Plan::sched
 #define U1_SVD_THREADS 128 // 4 warps per pair item, 6 CTAs per SM
 #define U1MPS_SORT_MAX 4096 // largest sector the in-smem bitonic sort takes (= U1MPS_CHI_MAX)
@@ -126,6 +127,7 @@ void u1_launch_contract(const DevState& S, const Plan& P, int G, const LaunchCfg
 cudaError_t u1_launch_svd(const DevState& S, const Plan& P, int G, const LaunchCfg& L);
 void u1_launch_select_scatter(const DevState& S, const Plan& P, int G, int chi, double cutoff, const LaunchCfg& L);
 void u1_launch_expect_n(const DevState& S, int site0, int nsites, double* part, int* count, double* out_dev, const LaunchCfg& L);
+cudaError_t u1_launch_expect_n_static(const DevState& S, int nsites, double* out_dev, const LaunchCfg& L);   // no allocation
 void u1_launch_entropy(const DevState& S, int bond0, int nbonds, double* out_dev, const LaunchCfg& L);
 void u1_launch_product_state(const DevState& S, const int* occ_dev, const LaunchCfg& L);
 void u1_launch_gamoff(const DevState& S, int site, const LaunchCfg& L);

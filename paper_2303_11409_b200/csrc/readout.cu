@@ -1,6 +1,7 @@
 // readout.cu — step a6 (canonical-form readouts, SURVEY §8(c) "Readouts"; Eq.10/15 canonical form)
 // and the small state-maintenance kernels (product state, block-offset rebuild after an import).
 #include <algorithm>
+#include <mutex>
 #include "common.cuh"
 
 #define RD_THREADS 256
@@ -200,4 +201,57 @@ void u1_launch_product_state(const DevState& S, const int* occ_dev, const Launch
 void u1_launch_gamoff(const DevState& S, int site, const LaunchCfg& L) {
   gamoff_kernel<<<1, 32, 0, L.stream>>>(S, site);
   ++*L.launches;
+}
+
+// ---- step a6 on library-owned static scratch: u1mps_expect_n_all_static (include/u1mps.h) --------------------------
+// The same expect_n_kernel, with the slice partial sums and the per-site slice counters in a file-scope device array
+// instead of the handle's arena, for callers that must not allocate (CUDA graph capture, serving loops): the call makes
+// no cudaMalloc / cudaFree and no allocating library call, only a memset node and one kernel launch on the handle's stream.
+// The array costs U1_RD_STATIC_BYTES (68 KiB) on every GPU that loads the library, until the process exits.  All handles
+// and all calls share it: two calls that overlap on the GPU (different streams, no ordering) race on it.  The counters
+// must start at zero, so every call clears the ones it uses first (the kernel also resets them when a site completes,
+// but a call that was aborted half way would otherwise poison the next one); the partial sums are written before read.
+#define U1_RD_STATIC_PART 8192                                                   // slice partial sums (doubles)
+#define U1_RD_STATIC_BYTES (U1_RD_STATIC_PART * 8 + U1_RD_STATIC_SITES * 4)      // + one counter per site = 69 632 bytes
+static __device__ __align__(256) unsigned char rd_static_scratch[U1_RD_STATIC_BYTES];
+
+#define U1_RD_MAXDEV 64
+// In host code `rd_static_scratch` is only the host-side shadow of the symbol, never a device address: the address
+// comes from cudaGetSymbolAddress, once per device, with that device current.
+static cudaError_t rd_static_address(unsigned char** out) {
+  static std::mutex mu;
+  static unsigned char* addr[U1_RD_MAXDEV] = {};
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= U1_RD_MAXDEV) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, rd_static_scratch);
+    if (e != cudaSuccess) return e;
+    addr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = addr[dev];
+  return cudaSuccess;
+}
+
+// nsites <= U1_RD_STATIC_SITES is the caller's check (api.cu turns a larger chain into U1MPS_ETOOBIG); out_dev: DEVICE
+// double[nsites], sites 0 .. nsites - 1.  Not timed by the stage profiler (its event pool may allocate).
+cudaError_t u1_launch_expect_n_static(const DevState& S, int nsites, double* out_dev, const LaunchCfg& L) {
+  if (nsites < 1 || nsites > U1_RD_STATIC_SITES) return cudaErrorInvalidValue;
+  unsigned char* base = nullptr;
+  cudaError_t e = rd_static_address(&base);
+  if (e != cudaSuccess) return e;
+  double* part = reinterpret_cast<double*>(base);
+  int* count = reinterpret_cast<int*>(base + (size_t)U1_RD_STATIC_PART * 8);
+  static int occ = 0;
+  if (occ == 0 && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, expect_n_kernel, RD_THREADS, 0) != cudaSuccess) occ = 4;
+  int K = std::max(1, std::min(U1_RD_SLICES, (std::max(occ, 1) * L.sms) / nsites));   // as u1_launch_expect_n ...
+  K = std::min(K, U1_RD_STATIC_PART / nsites);                                         // ... within the static array (>= 8)
+  e = cudaMemsetAsync(count, 0, (size_t)nsites * sizeof(int), L.stream);
+  if (e != cudaSuccess) return e;
+  expect_n_kernel<<<nsites * K, RD_THREADS, 0, L.stream>>>(S, 0, K, part, count, out_dev);
+  ++*L.launches;
+  return cudaGetLastError();
 }
