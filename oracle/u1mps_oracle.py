@@ -24,7 +24,8 @@ Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): P1 exact state vector (M<=
 invariants, P3 unit norm, P4 canonical-form identities, P5 Eckart-Young reconstruction, P6 brute
 force dense (non-symmetric) update Eq.11-14, P7 identity/swap gates, P8 closed forms (single
 particle walk, permanents, Hong-Ou-Mandel), P9 free-fermion <n_k>, P10 readout formula vs full
-environments, P11 tie order at the cut, P12 two-point <n_j n_k> vs the state vector.  Every function below is reached by at least one of them; nothing is
+environments, P11 tie order at the cut, P12 two-point <n_j n_k> vs the state vector, P13 Fock-pattern sampling vs conditional
+probabilities summed over the state vector.  Every function below is reached by at least one of them; nothing is
 "parity unpinned".
 """
 from __future__ import annotations
@@ -336,6 +337,72 @@ class U1MPS:
             if j < k and F is not None and cl in F:
                 val += (cl - cr) * float(np.real(np.trace(a.conj().T @ F[cl] @ a @ Rr[cr])))
         return val / norm
+
+    def sample_fock(self, u: np.ndarray):
+        """Fock patterns (n_0 .. n_{M-1}) drawn from |<n|psi>|^2 / <psi|psi>, site by site (pin P13).
+
+        The use the boson-sampling section motivates (Eq.7-8: the output distribution over occupation
+        patterns), on the state of Eq.15 (L112-114: the occupation of a site is the charge difference of its bonds).
+        The uniform numbers are an INPUT: u[b, s] in [0, 1) decides site s of sample b by inverse CDF over the
+        occupations in ascending order.  With A^[s](cl, cr) = Gamma^[s][cl, cr] diag(lambda^[s+1][cr]) and the right
+        environments R_M = {0: [[1]]}, R_s[cl] = sum_cr A R_{s+1}[cr] A^H (as in expect_n_full), a sample that has
+        reached bond s with charge c and boundary row vector v (v = [1] at bond 0) takes occupation i with weight
+            p_i = w_i R_{s+1}[c - i] w_i^H,   w_i = v A^[s](c, c - i),
+        chosen as the smallest i with u * sum_i' p_i' < p_0 + .. + p_i; then v <- w_i / sqrt(p_i), c <- c - i.
+        Exact for whatever Gamma, lambda the state holds (no canonical form assumed).
+
+        Returns (pattern int64 [B, M], logp float64 [B] = ln of the probability of the drawn pattern, margin float64
+        [B] = the smallest distance of u * sum p from a CDF step that was compared, relative to sum p: a draw with a
+        tiny margin is decided by rounding and is not comparable between implementations).
+        """
+        u = np.asarray(u, dtype=np.float64)
+        B, M = u.shape
+        assert M == self.M
+
+        def A(site, cl, cr):
+            return self.gam[site][(cl, cr)] * self.lam[site + 1][cr][None, :]
+        R = [None] * (M + 1)
+        R[M] = {0: np.ones((1, 1), dtype=np.complex128)}
+        for site in range(M - 1, -1, -1):
+            Rn: Dict[int, np.ndarray] = {}
+            for (cl, cr) in self.gam[site]:
+                if cr in R[site + 1]:
+                    a = A(site, cl, cr)
+                    Rn[cl] = Rn.get(cl, 0) + a @ R[site + 1][cr] @ a.conj().T
+            R[site] = Rn
+        pattern = np.zeros((B, M), dtype=np.int64)
+        logp = np.zeros(B)
+        margin = np.full(B, np.inf)
+        for b in range(B):
+            v = np.ones(1, dtype=np.complex128)
+            c = self.N
+            for site in range(M):
+                w = [None] * self.d
+                p = np.zeros(self.d)
+                for i in range(self.d):
+                    cr = c - i
+                    if (c, cr) in self.gam[site] and cr in R[site + 1]:
+                        w[i] = v @ A(site, c, cr)
+                        p[i] = float(np.real(w[i] @ R[site + 1][cr] @ w[i].conj()))
+                tot = 0.0
+                for i in range(self.d):
+                    tot += p[i]
+                target = u[b, site] * tot
+                cum, pick = 0.0, -1
+                for i in range(self.d):
+                    cum += p[i]
+                    if p[i] > 0.0:
+                        if pick < 0:
+                            margin[b] = min(margin[b], abs(target - cum) / tot)
+                        if pick < 0 and target < cum:
+                            pick = i
+                if pick < 0:                      # rounding at the top of the CDF: the last occupation with weight
+                    pick = max(i for i in range(self.d) if p[i] > 0.0)
+                pattern[b, site] = pick
+                logp[b] += math.log(p[pick] / tot)
+                v = w[pick] / math.sqrt(p[pick])
+                c -= pick
+        return pattern, logp, margin
 
     def to_dense(self):
         """Expand to a plain (non-symmetric) Vidal MPS: Gamma^[s]i (d, D_s, D_{s+1}), lambda^[k] (pin P6)."""

@@ -460,3 +460,63 @@ def test_P12_two_point_function_matches_state_vector():
                 ref = float(np.sum(p * digits[:, j] * digits[:, k]))
                 assert abs(st.expect_nn_full(j, k) - ref) < 1e-12, (chi, j, k)
         assert abs(sum(st.expect_nn_full(j, k) * (1 if j == k else 2) for j in range(M) for k in range(j, M)) - N * N) < 1e-10
+
+
+# ------------------------------------------------------------------ P13: Fock-pattern sampling
+def _brute_force_sampling(vec, d, M, u):
+    """Site-by-site inverse-CDF sampling straight from the d^M amplitudes: the conditional weight of occupation i at site
+    s given the prefix is the sum of |amplitude|^2 over all suffixes (site 0 = most significant digit, S23)."""
+    P = (np.abs(vec) ** 2).reshape((d,) * M)
+    total = P.sum()
+    pats, logps, margins = [], [], []
+    for b in range(u.shape[0]):
+        sub, pat, margin = P, [], np.inf
+        for s in range(M):
+            w = sub.reshape(d, -1).sum(axis=1)
+            target, cum, pick = u[b, s] * w.sum(), 0.0, -1
+            for i in range(d):
+                cum += w[i]
+                if w[i] > 0.0 and pick < 0:
+                    margin = min(margin, abs(target - cum) / w.sum())
+                    if target < cum:
+                        pick = i
+            if pick < 0:
+                pick = max(i for i in range(d) if w[i] > 0.0)
+            pat.append(pick)
+            sub = sub[pick]
+        pats.append(pat); logps.append(math.log(float(sub) / total)); margins.append(margin)
+    return np.array(pats), np.array(logps), np.array(margins)
+
+
+def test_P13_fock_sampling_matches_conditionals_of_the_state_vector():
+    """sample_fock against brute-force conditional sampling over the state vector with the same uniform numbers, on an
+    untruncated and on a truncated (non-canonical) state: same patterns, ln P(pattern) = ln(|<n|psi>|^2 / <psi|psi>);
+    every drawn pattern conserves the particle number; a product state always returns its own pattern."""
+    rng = np.random.default_rng(131)
+    d, M, N = 3, 6, 5
+    occ = [2, 0, 1, 1, 0, 1]
+    gates = brick_gates(rng, M, d, 3, lambda r: inputs.random_u1_gate(r, d))
+    u = rng.random((200, M))
+    for chi in (d ** 3, 4):
+        st = U1MPS.product_state(M, d, N, chi, occ)
+        for s, U in gates:
+            st.apply_gate(s, U, chi=chi, cutoff=1e-12)
+        if chi == 4:
+            assert st.discarded_total > 1e-4                      # the truncated state is not canonical any more
+        pat, logp, margin = st.sample_fock(u)
+        ref_pat, ref_logp, ref_margin = _brute_force_sampling(st.amplitudes(), d, M, u)
+        safe = np.minimum(margin, ref_margin) > 1e-9
+        assert safe.sum() >= 198
+        assert np.array_equal(pat[safe], ref_pat[safe]), chi
+        assert np.max(np.abs(logp[safe] - ref_logp[safe])) < 1e-10
+        assert np.all(pat.sum(axis=1) == N)
+        assert len({tuple(r) for r in pat}) > 20                    # a spread-out distribution, not one pattern
+        # the empirical frequencies follow the distribution: chi-square-free check on the first site's marginal
+        P0 = (np.abs(st.amplitudes()) ** 2).reshape(d, -1).sum(axis=1)
+        P0 = P0 / P0.sum()
+        big = U1MPS.sample_fock(st, rng.random((4000, M)))[0]
+        freq = np.bincount(big[:, 0], minlength=d) / 4000.0
+        assert np.max(np.abs(freq - P0)) < 5.0 * np.sqrt(0.25 / 4000.0)
+    prod = U1MPS.product_state(M, d, N, 4, occ)
+    pat, logp, _ = prod.sample_fock(rng.random((5, M)))
+    assert np.array_equal(pat, np.tile(occ, (5, 1))) and np.all(np.abs(logp) < 1e-14)
