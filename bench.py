@@ -358,9 +358,17 @@ def measure(w, args, steps, warmup, prep_columns, with_e2e, rank, world, local, 
         n_full = gpu.expect_n_full()
         full = {"sum_n_full": float(np.sum(n_full)), "max_abs_diff_to_canonical": float(np.max(np.abs(n_full - n_k))),
                 "seconds": time.perf_counter() - t0}
+    fock = None
+    if with_e2e:   # Fock-pattern sampling: 256 patterns from seeded uniform numbers, timed once
+        u = np.random.default_rng(20230311).random((256, w.M))
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        pat, logp = gpu.sample_fock(u)
+        fock = {"samples": 256, "seconds": time.perf_counter() - t0, "all_patterns_conserve_N": bool(np.all(pat.sum(axis=1) == w.N)),
+                "mean_log_prob": float(np.mean(logp)), "distinct_patterns": int(len({bytes(r) for r in pat}))}
     res = {"w": w, "ms": ms, "ms_e2e": ms_e2e, "launches": launches, "prof": prof, "clocks": clocks, "work": work,
            "work_after": work_after, "gates_per_step": gates_per_step, "prep_ms": prep_ms, "prep_gates": prep_gates,
-           "n_prep": n_prep, "stats": stats, "sum_n": float(np.sum(n_k)), "log_norm": ln, "a6": a6, "steps": steps, "full": full}
+           "n_prep": n_prep, "stats": stats, "sum_n": float(np.sum(n_k)), "log_norm": ln, "a6": a6, "steps": steps, "full": full, "fock": fock}
     gpu.close()
     del gpu, dev_cols, pin_cols
     torch.cuda.empty_cache()
@@ -517,7 +525,7 @@ def run_ours(args, w):
         "trajectory": {"gates": res["prep_gates"], "ms": res["prep_ms"],
                        "gates_per_s": res["prep_gates"] / (res["prep_ms"] * 1e-3) if res["prep_ms"] > 0 else None},
         "state": {"sum_n": res["sum_n"], "log_norm": res["log_norm"], "discarded": stats["discarded"], "svd_sweeps_max": stats["sweeps"],
-                  "svd_converged": stats["converged"], "full_environment_readout": res["full"]},
+                  "svd_converged": stats["converged"], "full_environment_readout": res["full"], "fock_sampling": res["fock"]},
         "cpu_baseline": cpu,
         "per_workload": per_workload,
     }

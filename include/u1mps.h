@@ -137,6 +137,19 @@ int u1mps_expect_n_full(u1mps_t* h, double* out_host, void* scratch_dev, size_t 
  * scratch of at least u1mps_expect_nn_full_bytes (six environment-sized and two Gamma-sized buffers).  Both [sync]. */
 int u1mps_expect_nn_full_bytes(u1mps_t* h, size_t* bytes_host);
 int u1mps_expect_nn_full(u1mps_t* h, int site_j, int site_k, double* out_host, void* scratch_dev, size_t scratch_bytes);
+/* Fock-pattern sampling (Eq.7-8: the distribution over occupation patterns that
+ * boson sampling asks for; state of Eq.15): n_samples patterns (n_0 .. n_{M-1}), each drawn from
+ * |<n|psi>|^2 / <psi|psi> exactly (right environments contracted explicitly, so truncation does not bias the draw).
+ * The random numbers are an INPUT: u_host[b * M + s] in [0, 1) (else U1MPS_EINVAL) decides site s of sample b by inverse
+ * CDF over the occupations 0 .. d-1 in ascending order, conditioned on the occupations already drawn for sites < s; the
+ * same u gives the same patterns on every run.  pattern_host: HOST int32 [n_samples * M]; logp_host: HOST [n_samples],
+ * ln of the probability of the drawn pattern.  Device scratch (256-byte aligned) of at least u1mps_sample_fock_bytes:
+ * all right environments of the chain (sum over bonds and sectors of n^2 complex128), one Gamma-sized buffer and
+ * (d + 2) boundary vectors per sample; U1MPS_ENOMEM if it is too small.  1 <= n_samples <= U1MPS_SAMPLES_MAX.  Both [sync]. */
+#define U1MPS_SAMPLES_MAX 65536
+int u1mps_sample_fock_bytes(u1mps_t* h, int n_samples, size_t* bytes_host);
+int u1mps_sample_fock(u1mps_t* h, int n_samples, const double* u_host, int32_t* pattern_host, double* logp_host,
+                      void* scratch_dev, size_t scratch_bytes);
 /* Sector table of a bond: writes up to cap (charge, count) pairs, ascending charge; *n_sectors = how many exist. */
 int u1mps_bond_info(u1mps_t* h, int bond, int32_t* n_sectors, int32_t* charges, int32_t* counts, int cap);
 int u1mps_bond_dims(u1mps_t* h, int32_t* dims_host /*[M+1]*/);

@@ -24,6 +24,7 @@ EXPORTS = [
     "u1mps_export_staged_svd", "u1mps_launch_count", "u1mps_profile_enable", "u1mps_profile_read",
     "u1mps_stage_name", "u1mps_svd_trace", "u1mps_clear_status", "u1mps_expect_n_full_bytes", "u1mps_expect_n_full",
     "u1mps_expect_nn_full_bytes", "u1mps_expect_nn_full", "u1mps_expect_n_all_static",
+    "u1mps_sample_fock_bytes", "u1mps_sample_fock",
 ]
 NSTAGE = 8
 
@@ -92,6 +93,8 @@ def load_library() -> C.CDLL:
     lib.u1mps_expect_nn_full_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     lib.u1mps_expect_nn_full.argtypes = [vp, C.c_int, C.c_int, dp, vp, C.c_size_t]
     lib.u1mps_expect_n_all_static.argtypes = [vp, vp]
+    lib.u1mps_sample_fock_bytes.argtypes = [vp, C.c_int, C.POINTER(C.c_size_t)]
+    lib.u1mps_sample_fock.argtypes = [vp, C.c_int, dp, i32p, dp, vp, C.c_size_t]
     lib.u1mps_stage_name.restype = C.c_char_p
     lib.u1mps_stage_name.argtypes = [C.c_int]
     for name in EXPORTS:
@@ -223,6 +226,23 @@ class U1MPS:
                 and out_dev.is_contiguous() and out_dev.numel() >= self.M):
             raise U1MPSError(-1, "out_dev must be a contiguous CUDA float64 tensor of at least M elements")
         self._ck(self.lib.u1mps_expect_n_all_static(self.h, C.c_void_p(out_dev.data_ptr())))
+
+    def sample_fock(self, u) -> Tuple[np.ndarray, np.ndarray]:
+        """Fock patterns drawn from |<n|psi>|^2 / <psi|psi>; u: [B, M] uniform numbers in [0, 1) (the caller's random
+        numbers).  Returns (pattern int32 [B, M], logp [B])."""
+        import torch
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        if u.ndim != 2 or u.shape[1] != self.M:
+            raise U1MPSError(-1, "u must be [n_samples, M]")
+        B = u.shape[0]
+        nbytes = C.c_size_t()
+        self._ck(self.lib.u1mps_sample_fock_bytes(self.h, B, C.byref(nbytes)))
+        scratch = torch.empty(max(nbytes.value, 256), dtype=torch.uint8, device="cuda")
+        pat = np.zeros((B, self.M), dtype=np.int32)
+        logp = np.zeros(B)
+        self._ck(self.lib.u1mps_sample_fock(self.h, B, _ptr(u, C.POINTER(C.c_double)), _ptr(pat, C.POINTER(C.c_int32)),
+                                            _ptr(logp, C.POINTER(C.c_double)), C.c_void_p(scratch.data_ptr()), nbytes.value))
+        return pat, logp
 
     def expect_n_full(self) -> np.ndarray:
         """<psi|n_k|psi> / <psi|psi> with explicit environments (exact also after truncation); scratch from torch."""

@@ -515,6 +515,34 @@ int u1mps_expect_nn_full(u1mps_t* h, int site_j, int site_k, double* out, void* 
   return U1MPS_OK;
 }
 
+int u1mps_sample_fock_bytes(u1mps_t* h, int n_samples, size_t* bytes) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
+  if (!h || !bytes || n_samples < 1 || n_samples > U1MPS_SAMPLES_MAX) return U1MPS_EINVAL;
+  if (h->stage != ST_NONE) return U1MPS_ESTAGED;
+  std::vector<long long> gamoff, gused;
+  int r = env_tables(h, gamoff, gused);
+  if (r) return r;
+  *bytes = u1_env_sample_scratch_bytes(h->M, h->NC, h->d, h->h_nb, gused, n_samples);
+  return U1MPS_OK;
+}
+
+int u1mps_sample_fock(u1mps_t* h, int n_samples, const double* u, int32_t* pattern, double* logp, void* scratch_dev, size_t scratch_bytes) {
+  if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
+  if (!h || !u || !pattern || !logp || !scratch_dev || ((uintptr_t)scratch_dev & 255) || n_samples < 1 || n_samples > U1MPS_SAMPLES_MAX)
+    return U1MPS_EINVAL;
+  for (long long x = 0; x < (long long)n_samples * h->M; ++x)
+    if (!(u[x] >= 0.0 && u[x] < 1.0)) return U1MPS_EINVAL;   // also rejects NaN
+  if (h->stage != ST_NONE) return U1MPS_ESTAGED;
+  std::vector<long long> gamoff, gused;
+  int r = env_tables(h, gamoff, gused);
+  if (r) return r;
+  if (scratch_bytes < u1_env_sample_scratch_bytes(h->M, h->NC, h->d, h->h_nb, gused, n_samples)) return U1MPS_ENOMEM;
+  static_assert(sizeof(int32_t) == sizeof(int), "pattern buffer");
+  CK(u1_env_sample_fock(h->S, h->h_nb, gamoff, gused, n_samples, u, reinterpret_cast<int*>(pattern), logp, scratch_dev, h->L));
+  CK(cudaStreamSynchronize(h->stream));
+  return U1MPS_OK;
+}
+
 int u1mps_bond_entropy_all(u1mps_t* h, double* out) {
   if (h && h->cuda_err != cudaSuccess) return U1MPS_ECUDA;   // sticky
   if (!h || !out) return U1MPS_EINVAL;

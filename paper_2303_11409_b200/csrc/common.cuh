@@ -136,5 +136,9 @@ size_t u1_env_scratch_bytes(int M, int NC, int d, const std::vector<int>& nb, co
 size_t u1_env_nn_scratch_bytes(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused);
 cudaError_t u1_env_expect_nn(const DevState& S, const std::vector<int>& nb, const std::vector<long long>& gamoff,
                              const std::vector<long long>& gused, int j, int k, void* scratch, double* out_dev, const LaunchCfg& L);
+size_t u1_env_sample_scratch_bytes(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused, int B);
+cudaError_t u1_env_sample_fock(const DevState& S, const std::vector<int>& nb, const std::vector<long long>& gamoff,
+                               const std::vector<long long>& gused, int B, const double* u_host, int* pat_host, double* logp_host,
+                               void* scratch, const LaunchCfg& L);
 cudaError_t u1_env_expect_n(const DevState& S, const std::vector<int>& nb, const std::vector<long long>& gamoff,
                             const std::vector<long long>& gused, void* scratch, double* out_dev, const LaunchCfg& L);

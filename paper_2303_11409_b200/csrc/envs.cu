@@ -544,3 +544,278 @@ cudaError_t u1_env_expect_nn(const DevState& S, const std::vector<int>& nb, cons
   ++*L.launches;
   return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Fock-pattern sampling (the output distribution over occupation patterns; state
+// of Eq.15): patterns drawn from |<n|psi>|^2 / <psi|psi> site by site, exactly, for whatever Gamma, lambda the
+// handle holds.  All right environments R_s[cl] = sum_cr A R_{s+1}[cr] A^H are built once by the grouped GEMMs above and
+// kept; then one launch per site advances every sample: a sample at bond s with charge c and boundary row vector v takes
+// occupation i with weight p_i = w_i R_{s+1}[c - i] w_i^H, w_i = v Gamma^[s][c, c - i] diag(lambda^[s+1][c - i]), by
+// inverse CDF on the uniform number the caller passed for (sample, site); v <- w_i / sqrt(p_i), c <- c - i.
+// One CTA per sample; the vector-matrix products split the inner index over the 8 warps and the output index over the
+// lanes (coalesced rows), partial sums added in warp order: results do not depend on timing.
+#define FS_THREADS 256
+#define FS_WARPS (FS_THREADS / 32)
+#define FS_BC 256   // output columns per pass (8 per lane)
+
+// out[b] = sc[b] * sum_a v[a] Mt[a * n_out + b]  (store != nullptr), or the return value (valid in every thread)
+// Re sum_b (sum_a v[a] Mt[a * n_out + b]) conj(wref[b])  (store == nullptr)
+__device__ double fs_vecmat(const cplx* __restrict__ v, int n_in, const cplx* __restrict__ Mt, int n_out, const double* __restrict__ sc,
+                            cplx* store, const cplx* wref, cplx* part, double* red) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int a0 = (int)((long long)n_in * warp / FS_WARPS), a1 = (int)((long long)n_in * (warp + 1) / FS_WARPS);
+  double dacc = 0.0;
+  for (int b0 = 0; b0 < n_out; b0 += FS_BC) {
+    double ar[FS_BC / 32], ai[FS_BC / 32];
+#pragma unroll
+    for (int x = 0; x < FS_BC / 32; ++x) { ar[x] = 0.0; ai[x] = 0.0; }
+    for (int a = a0; a < a1; ++a) {
+      const cplx va = v[a];
+      const cplx* row = Mt + (long long)a * n_out + b0 + lane;
+#pragma unroll
+      for (int x = 0; x < FS_BC / 32; ++x) {
+        if (b0 + lane + 32 * x < n_out) {
+          const cplx g = row[32 * x];
+          ar[x] = fma(va.x, g.x, fma(-va.y, g.y, ar[x]));
+          ai[x] = fma(va.x, g.y, fma(va.y, g.x, ai[x]));
+        }
+      }
+    }
+#pragma unroll
+    for (int x = 0; x < FS_BC / 32; ++x) part[warp * FS_BC + lane + 32 * x] = make_double2(ar[x], ai[x]);
+    __syncthreads();
+    if (b0 + tid < n_out) {   // FS_THREADS == FS_BC: one output column per thread
+      double tr = 0.0, ti = 0.0;
+#pragma unroll
+      for (int w = 0; w < FS_WARPS; ++w) { const cplx q = part[w * FS_BC + tid]; tr += q.x; ti += q.y; }
+      if (store) {
+        const double s = sc ? sc[b0 + tid] : 1.0;
+        store[b0 + tid] = make_double2(tr * s, ti * s);
+      } else {
+        const cplx r = wref[b0 + tid];
+        dacc = fma(tr, r.x, fma(ti, r.y, dacc));
+      }
+    }
+    __syncthreads();
+  }
+  if (store) return 0.0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) dacc += __shfl_xor_sync(0xffffffffu, dacc, o);
+  if (lane == 0) red[warp] = dacc;
+  __syncthreads();
+  double t = 0.0;
+#pragma unroll
+  for (int w = 0; w < FS_WARPS; ++w) t += red[w];
+  __syncthreads();
+  return t;
+}
+static_assert(FS_THREADS == FS_BC, "fs_vecmat: one output column per thread");
+
+__global__ void __launch_bounds__(FS_THREADS) fock_step_kernel(DevState S, int s, const cplx* __restrict__ Rall, const long long* __restrict__ roff,
+                                                               const double* __restrict__ u, const cplx* __restrict__ vcur, cplx* vnext, cplx* wbuf,
+                                                               int* cs, int* pat, double* logp, int maxn) {
+  __shared__ __align__(16) cplx part[FS_WARPS * FS_BC];
+  __shared__ double red[FS_WARPS];
+  __shared__ double s_p[EV_MAXTERM];
+  __shared__ int s_pick;
+  __shared__ double s_scale;
+  const int b = blockIdx.x, tid = threadIdx.x, NC = S.NC, d = S.d, M = S.M;
+  const int c = cs[b];
+  const int* nbL = S.nb + (long long)s * NC;
+  const int* nbR = S.nb + (long long)(s + 1) * NC;
+  const int nl = nbL[c];
+  const cplx* v = vcur + (long long)b * maxn;
+  const cplx* gam = S.gam + (long long)s * S.gcap;
+  const long long* goff = S.gamoff + (long long)s * NC * d;
+  for (int i = 0; i < d; ++i) {
+    const int cr = c - i;
+    double p = 0.0;
+    const int nr = cr >= 0 ? nbR[cr] : 0;
+    if (nr > 0 && nl > 0) {   // uniform over the CTA
+      cplx* w = wbuf + ((long long)b * d + i) * maxn;
+      fs_vecmat(v, nl, gam + goff[c * d + i], nr, S.lam + (long long)(s + 1) * S.chi + S.ob[(long long)(s + 1) * NC + cr], w, nullptr, part, red);
+      __syncthreads();   // w (global) is read back by other threads of the CTA
+      p = fs_vecmat(w, nr, Rall + roff[(long long)(s + 1) * NC + cr], nr, nullptr, nullptr, w, part, red);
+    }
+    if (tid == 0) s_p[i] = p;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double tot = 0.0;
+    for (int i = 0; i < d; ++i) tot += s_p[i];
+    const double target = u[(long long)b * M + s] * tot;
+    double cum = 0.0;
+    int pick = -1, last = 0;
+    for (int i = 0; i < d; ++i) {
+      cum += s_p[i];
+      if (s_p[i] > 0.0) { last = i; if (pick < 0 && target < cum) pick = i; }
+    }
+    if (pick < 0) pick = last;   // rounding at the top of the CDF
+    pat[(long long)b * M + s] = pick;
+    logp[b] += log(s_p[pick] / tot);
+    cs[b] = c - pick;
+    s_pick = pick;
+    s_scale = rsqrt(s_p[pick]);
+  }
+  __syncthreads();
+  const int pick = s_pick;
+  const int nrp = (c - pick >= 0) ? nbR[c - pick] : 0;
+  const double sc = s_scale;
+  const cplx* w = wbuf + ((long long)b * d + pick) * maxn;
+  cplx* vn = vnext + (long long)b * maxn;
+  for (int x = tid; x < nrp; x += FS_THREADS) { const cplx q = w[x]; vn[x] = make_double2(q.x * sc, q.y * sc); }
+}
+
+__global__ void fock_init_kernel(int B, int N, int maxn, cplx* vcur, int* cs, double* logp) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= B) return;
+  vcur[(long long)b * maxn] = make_double2(1.0, 0.0);
+  cs[b] = N;
+  logp[b] = 0.0;
+}
+
+namespace {
+struct FockLayout {
+  EnvLayout E;          // Ebase / eoff / Etot / maxG (its own offsets are not used here)
+  int maxn = 1;
+  size_t ndesc = 0, npref = 0;
+  size_t o_desc = 0, o_pref = 0, o_R = 0, o_S = 0, o_roff = 0, o_u = 0, o_pat = 0, o_logp = 0, o_cs = 0, o_v0 = 0, o_v1 = 0, o_w = 0, total = 0;
+};
+FockLayout fock_layout(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused, int B) {
+  FockLayout Y;
+  Y.E = env_layout(M, NC, d, nb, gused);
+  for (size_t x = 0; x < nb.size(); ++x) Y.maxn = std::max(Y.maxn, nb[x]);
+  for (int s = 0; s < M; ++s) {
+    size_t nblk = 0, nL = 0;
+    for (int cl = 0; cl < NC; ++cl) {
+      if (nb[(size_t)s * NC + cl]) ++nL;
+      for (int i = 0; i < d && cl - i >= 0; ++i)
+        if (nb[(size_t)s * NC + cl] && nb[(size_t)(s + 1) * NC + cl - i]) ++nblk;
+    }
+    Y.ndesc += nblk + nL;
+    Y.npref += nblk + nL + 2;
+  }
+  size_t o = 0;
+  Y.o_desc = o; o = al256(o + Y.ndesc * sizeof(EnvDesc));
+  Y.o_pref = o; o = al256(o + Y.npref * sizeof(int));
+  Y.o_R = o;    o = al256(o + (size_t)Y.E.Etot * sizeof(cplx));
+  Y.o_S = o;    o = al256(o + (size_t)Y.E.maxG * sizeof(cplx));
+  Y.o_roff = o; o = al256(o + (size_t)(M + 1) * NC * sizeof(long long));
+  Y.o_u = o;    o = al256(o + (size_t)B * M * sizeof(double));
+  Y.o_pat = o;  o = al256(o + (size_t)B * M * sizeof(int));
+  Y.o_logp = o; o = al256(o + (size_t)B * sizeof(double));
+  Y.o_cs = o;   o = al256(o + (size_t)B * sizeof(int));
+  Y.o_v0 = o;   o = al256(o + (size_t)B * Y.maxn * sizeof(cplx));
+  Y.o_v1 = o;   o = al256(o + (size_t)B * Y.maxn * sizeof(cplx));
+  Y.o_w = o;    o = al256(o + (size_t)B * d * Y.maxn * sizeof(cplx));
+  Y.total = o;
+  return Y;
+}
+}  // namespace
+
+size_t u1_env_sample_scratch_bytes(int M, int NC, int d, const std::vector<int>& nb, const std::vector<long long>& gused, int B) {
+  return fock_layout(M, NC, d, nb, gused, B).total;
+}
+
+// Host driver.  u_host: HOST [B * M] uniform numbers in [0, 1); pat_host: HOST int32 [B * M]; logp_host: HOST [B] (ln of
+// the probability of the drawn pattern).  Everything is enqueued on L.stream; the caller synchronises.
+cudaError_t u1_env_sample_fock(const DevState& S, const std::vector<int>& nb, const std::vector<long long>& gamoff,
+                               const std::vector<long long>& gused, int B, const double* u_host, int* pat_host, double* logp_host,
+                               void* scratch, const LaunchCfg& L) {
+  const int M = S.M, NC = S.NC, d = S.d;
+  const FockLayout Y = fock_layout(M, NC, d, nb, gused, B);
+  char* base = (char*)scratch;
+  EnvDesc* d_desc = (EnvDesc*)(base + Y.o_desc);
+  int* d_pref = (int*)(base + Y.o_pref);
+  cplx* Rall = (cplx*)(base + Y.o_R);
+  cplx* Sbuf = (cplx*)(base + Y.o_S);
+  long long* d_roff = (long long*)(base + Y.o_roff);
+  double* d_u = (double*)(base + Y.o_u);
+  int* d_pat = (int*)(base + Y.o_pat);
+  double* d_logp = (double*)(base + Y.o_logp);
+  int* d_cs = (int*)(base + Y.o_cs);
+  cplx* v0 = (cplx*)(base + Y.o_v0);
+  cplx* v1 = (cplx*)(base + Y.o_v1);
+  cplx* wbuf = (cplx*)(base + Y.o_w);
+  std::vector<int> ob((size_t)(M + 1) * NC);
+  std::vector<long long> roff((size_t)(M + 1) * NC);
+  for (int k = 0; k <= M; ++k) {
+    int run = 0;
+    for (int c = 0; c < NC; ++c) {
+      ob[(size_t)k * NC + c] = run; run += nb[(size_t)k * NC + c];
+      roff[(size_t)k * NC + c] = Y.E.Ebase[k] + Y.E.eoff[(size_t)k * NC + c];
+    }
+  }
+  auto nK = [&](int k, int c) { return nb[(size_t)k * NC + c]; };
+  auto Rptr = [&](int k, int c) { return Rall + roff[(size_t)k * NC + c]; };
+  auto lamp = [&](int k, int c) { return S.lam + (size_t)k * S.chi + ob[(size_t)k * NC + c]; };
+  auto goff = [&](int s, int cl, int i) { return gamoff[((size_t)s * NC + cl) * d + i]; };
+  struct Launch { size_t d0, p0; int nd, tiles; };
+  std::vector<EnvDesc> descs; descs.reserve(Y.ndesc);
+  std::vector<int> prefs; prefs.reserve(Y.npref);
+  std::vector<Launch> LA((size_t)M * 2);   // per site: R1, R2
+  auto begin_launch = [&](Launch& la) { la.d0 = descs.size(); la.p0 = prefs.size(); la.nd = 0; la.tiles = 0; prefs.push_back(0); };
+  auto push = [&](Launch& la, const EnvDesc& D) {
+    descs.push_back(D);
+    la.tiles += u1_ceil_div(D.m, U1_TILE) * u1_ceil_div(D.n, U1_TILE);
+    prefs.push_back(la.tiles);
+    ++la.nd;
+  };
+  EnvDesc Z;
+  for (int t = 0; t < EV_MAXTERM; ++t) { Z.A[t] = nullptr; Z.B[t] = nullptr; Z.ks[t] = nullptr; Z.k[t] = 0; Z.w[t] = 1.0; }
+  Z.C = nullptr; Z.rs = nullptr; Z.cs = nullptr; Z.alpha = 1.0; Z.m = Z.n = Z.nterm = Z.opA = Z.opB = 0;
+  for (int s = 0; s < M; ++s) {
+    const cplx* G = S.gam + (size_t)s * S.gcap;
+    Launch &r1 = LA[(size_t)s * 2], &r2 = LA[(size_t)s * 2 + 1];
+    begin_launch(r1);   // S_f = Gamma_f lam R_{s+1}[cr] lam
+    for (int cl = 0; cl < NC; ++cl) for (int i = 0; i < d && cl - i >= 0; ++i) {
+      const int nl = nK(s, cl), nr = nK(s + 1, cl - i);
+      if (!nl || !nr) continue;
+      EnvDesc D = Z; D.m = nl; D.n = nr; D.nterm = 1; D.A[0] = G + goff(s, cl, i); D.ks[0] = lamp(s + 1, cl - i); D.B[0] = Rptr(s + 1, cl - i);
+      D.k[0] = nr; D.cs = lamp(s + 1, cl - i); D.C = Sbuf + goff(s, cl, i);
+      push(r1, D);
+    }
+    begin_launch(r2);   // R_s[cl] = sum_i S_f Gamma_f^H
+    for (int cl = 0; cl < NC; ++cl) {
+      const int nl = nK(s, cl);
+      if (!nl) continue;
+      EnvDesc D = Z; D.m = nl; D.n = nl; D.opB = 1; D.C = Rptr(s, cl);
+      for (int i = 0; i < d && cl - i >= 0; ++i) {
+        const int nr = nK(s + 1, cl - i);
+        if (!nr) continue;
+        D.A[D.nterm] = Sbuf + goff(s, cl, i); D.B[D.nterm] = G + goff(s, cl, i); D.k[D.nterm] = nr; ++D.nterm;
+      }
+      push(r2, D);   // (no term: a dead-end sector - zero environment, no sample can enter it)
+    }
+  }
+  if (descs.size() > Y.ndesc || prefs.size() > Y.npref) return cudaErrorInvalidValue;
+  cudaError_t err;
+  if ((err = cudaMemcpyAsync(d_desc, descs.data(), descs.size() * sizeof(EnvDesc), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemcpyAsync(d_pref, prefs.data(), prefs.size() * sizeof(int), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemcpyAsync(d_roff, roff.data(), roff.size() * sizeof(long long), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemcpyAsync(d_u, u_host, (size_t)B * M * sizeof(double), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  if ((err = cudaMemsetAsync(Rall, 0, (size_t)Y.E.Etot * sizeof(cplx), L.stream)) != cudaSuccess) return err;
+  const cplx one = make_double2(1.0, 0.0);
+  if ((err = cudaMemcpyAsync(Rptr(M, 0), &one, sizeof(cplx), cudaMemcpyHostToDevice, L.stream)) != cudaSuccess) return err;
+  auto run = [&](const Launch& la) {
+    if (la.tiles == 0) return;
+    L.prof->begin(U1_ST_READOUT, L.stream);
+    env_gemm_kernel<<<std::min(la.tiles, L.sms * 8), EV_THREADS, 0, L.stream>>>(d_desc + la.d0, d_pref + la.p0, la.nd);
+    L.prof->end(L.stream);
+    ++*L.launches;
+  };
+  for (int s = M - 1; s >= 0; --s) { run(LA[(size_t)s * 2]); run(LA[(size_t)s * 2 + 1]); }
+  fock_init_kernel<<<u1_ceil_div(B, 256), 256, 0, L.stream>>>(B, S.N, Y.maxn, v0, d_cs, d_logp);
+  ++*L.launches;
+  cplx *vc = v0, *vn = v1;
+  for (int s = 0; s < M; ++s) {
+    L.prof->begin(U1_ST_READOUT, L.stream);
+    fock_step_kernel<<<B, FS_THREADS, 0, L.stream>>>(S, s, Rall, d_roff, d_u, vc, vn, wbuf, d_cs, d_pat, d_logp, Y.maxn);
+    L.prof->end(L.stream);
+    ++*L.launches;
+    std::swap(vc, vn);
+  }
+  if ((err = cudaGetLastError()) != cudaSuccess) return err;
+  if ((err = cudaMemcpyAsync(pat_host, d_pat, (size_t)B * M * sizeof(int), cudaMemcpyDeviceToHost, L.stream)) != cudaSuccess) return err;
+  return cudaMemcpyAsync(logp_host, d_logp, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, L.stream);
+}

@@ -212,6 +212,53 @@ def test_expect_nn_full_on_truncated_states(idx, M, N, chi, cols):
     assert gpu.expect_nn_full(3, 1) == gpu.expect_nn_full(1, 3)
 
 
+@pytest.mark.parametrize("idx,M,N,chi,cols,B", [
+    (2, 16, 8, 12, 14, 300),    # hard truncation (non-canonical state)
+    (3, 20, 10, 6, 40, 300),
+    (4, 8, 4, 6, 8, 300),       # d = 5
+    (5, 10, 5, 6, 10, 300),     # d = 4
+    (2, 22, 11, 1200, 14, 48),  # sectors of more than 256 columns: several passes of the vector-matrix product
+])
+def test_sample_fock_matches_the_oracle(idx, M, N, chi, cols, B):
+    """u1mps_sample_fock against the oracle's sample_fock (pinned by P13 against conditional sampling over the state
+    vector) with the same uniform numbers: identical patterns wherever the oracle's decision margin is not at rounding
+    level (a draw whose u * sum p sits within 1e-9 of a CDF step is decided by rounding), ln P(pattern) to 1e-9,
+    every pattern conserves the particle number, and the same u gives the same patterns again."""
+    w = inputs.small_variant(inputs.WORKLOADS[idx], M=M, N=N, chi=chi, columns=cols)
+    ora, gpu = run_both(w)
+    if chi == 1200:
+        assert max(len(v) for k in range(w.M + 1) for v in ora.lam[k].values()) > 256
+    u = np.random.default_rng(1000 + idx).random((B, w.M))
+    want_pat, want_logp, margin = ora.sample_fock(u)
+    got_pat, got_logp = gpu.sample_fock(u)
+    safe = margin > 1e-9
+    print(f"sample_fock config {idx}: {int((~safe).sum())} of {B} draws at rounding level")
+    assert safe.sum() >= B - 2
+    assert np.array_equal(got_pat[safe], want_pat[safe])
+    assert np.max(np.abs(got_logp[safe] - want_logp[safe])) <= 1e-9
+    assert np.all(got_pat.sum(axis=1) == w.N)
+    assert np.all((got_pat >= 0) & (got_pat < w.d))
+    again_pat, again_logp = gpu.sample_fock(u)
+    assert np.array_equal(again_pat, got_pat) and np.array_equal(again_logp, got_logp)
+    # the state is untouched by the read-out
+    assert_observables(ora, gpu)
+
+
+def test_sample_fock_product_state_and_argument_checks():
+    from paper_2303_11409_b200.binding import U1MPSError
+    occ = [2, 0, 1, 2, 0, 0]
+    gpu = make_gpu(6, 3, 5, 8)
+    gpu.set_product_state(occ)
+    pat, logp = gpu.sample_fock(np.random.default_rng(5).random((7, 6)))
+    assert np.array_equal(pat, np.tile(occ, (7, 1))) and np.all(np.abs(logp) <= 1e-14)
+    for bad in (np.full((2, 6), 1.0), np.full((2, 6), -0.1), np.full((2, 6), np.nan)):
+        with pytest.raises(U1MPSError) as ei:
+            gpu.sample_fock(bad)
+        assert ei.value.code == -1
+    assert np.allclose(gpu.expect_n_all(), occ)
+
+
+
 # ------------------------------------------------------------------ the tie order at the cut (reading S8)
 def test_exact_tie_at_the_cut_and_keep_at_least_one():
     """An exact tie across two sectors at the cut: |10> under a gate with equal amplitudes to stay and to hop gives
