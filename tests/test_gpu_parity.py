@@ -244,6 +244,34 @@ def test_sample_fock_matches_the_oracle(idx, M, N, chi, cols, B):
     assert_observables(ora, gpu)
 
 
+def test_f4_readouts_on_the_full_config2_state():
+    """The full-environment read-outs at BASELINE.json's full size: config 2 (M = 64, chi = 256) run to the end of its own
+    40 columns on the device, the state exported and handed to the oracle (the teacher-forced protocol of SURVEY section
+    8(c)), and <n_k> (sampled sites), <n_j n_k> (sampled pairs) and Fock patterns (16 draws) compared on that state;
+    the properties that hold at any size for all sites: sum_k <n_k> = N, every pattern sums to N."""
+    w = inputs.WORKLOADS[2]
+    gpu = make_gpu(w.M, w.d, w.N, w.chi)
+    gpu.set_product_state(w.occ)
+    for sites, us in inputs.gate_columns(w):
+        gpu.apply_gate_column(sites, us, cutoff=w.cutoff)
+    assert gpu.last_stats()["converged"] and int(max(gpu.bond_dims())) == w.chi
+    ora = gpu_to_oracle(gpu)
+    n_full = gpu.expect_n_full()
+    assert abs(np.sum(n_full) - w.N) <= 1e-9
+    for k in (0, 17, 32, 63):
+        assert abs(n_full[k] - ora.expect_n_full(k)) <= 1e-9, k
+    for j, k in ((5, 5), (20, 41), (31, 32)):
+        assert abs(gpu.expect_nn_full(j, k) - ora.expect_nn_full(j, k)) <= 1e-9, (j, k)
+    u = np.random.default_rng(2002).random((16, w.M))
+    want_pat, want_logp, margin = ora.sample_fock(u)
+    got_pat, got_logp = gpu.sample_fock(u)
+    safe = margin > 1e-9
+    assert safe.sum() >= 15
+    assert np.array_equal(got_pat[safe], want_pat[safe])
+    assert np.max(np.abs(got_logp[safe] - want_logp[safe])) <= 1e-9
+    assert np.all(got_pat.sum(axis=1) == w.N)
+
+
 def test_sample_fock_product_state_and_argument_checks():
     from paper_2303_11409_b200.binding import U1MPSError
     occ = [2, 0, 1, 2, 0, 0]
