@@ -269,6 +269,21 @@ def readout_bytes(gpu, w):
     return by
 
 
+def env_flops(gpu, w):
+    """Useful flops of one u1mps_expect_n_full call: per site the five grouped complex GEMMs of csrc/envs.cu (E Gamma;
+    the same weighted by the occupation, for blocks with i >= 1; Gamma^H T; Gamma lam R lam; S Gamma^H), 8 real flops per
+    complex multiply-add, over the (cl, cr) blocks of the current sector tables."""
+    tabs = [dict(gpu.bond_info(k)) for k in range(w.M + 1)]
+    fl = 0
+    for s in range(w.M):
+        for cl, nl in tabs[s].items():
+            for i in range(w.d):
+                nr = tabs[s + 1].get(cl - i, 0)
+                if nr:
+                    fl += 8 * (nl * nl * nr * (2 if i else 1) + nr * nr * nl + nl * nr * nr + nl * nl * nr)
+    return fl
+
+
 def measure(w, args, steps, warmup, prep_columns, with_e2e, rank, world, local, barrier):
     """One workload on this rank's GPU: the config's own columns as preparation, then `steps` timed brick-wall layers."""
     import torch
@@ -358,6 +373,8 @@ def measure(w, args, steps, warmup, prep_columns, with_e2e, rank, world, local, 
         n_full = gpu.expect_n_full()
         full = {"sum_n_full": float(np.sum(n_full)), "max_abs_diff_to_canonical": float(np.max(np.abs(n_full - n_k))),
                 "seconds": time.perf_counter() - t0}
+        full["useful_tflops"] = env_flops(gpu, w) / full["seconds"] / 1e12   # wall clock of the whole call (table read-back,
+        full["note"] = "useful_tflops = five grouped complex128 GEMMs per site / wall time of the call"   # uploads, sync)
     fock = None
     if with_e2e:   # Fock-pattern sampling: 256 patterns from seeded uniform numbers, timed once
         u = np.random.default_rng(20230311).random((256, w.M))
