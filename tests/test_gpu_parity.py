@@ -283,6 +283,20 @@ def test_sample_fock_product_state_and_argument_checks():
         with pytest.raises(U1MPSError) as ei:
             gpu.sample_fock(bad)
         assert ei.value.code == -1
+    # scratch too small / misaligned: refused before anything is enqueued
+    import ctypes as C
+    import torch
+    u = np.ascontiguousarray(np.random.default_rng(6).random((2, 6)))
+    pat, lp = np.zeros((2, 6), np.int32), np.zeros(2)
+    need = C.c_size_t()
+    assert gpu.lib.u1mps_sample_fock_bytes(gpu.h, 2, C.byref(need)) == 0 and need.value > 256
+    buf = torch.empty(need.value + 512, dtype=torch.uint8, device="cuda")
+    args = (gpu.h, 2, u.ctypes.data_as(C.POINTER(C.c_double)), pat.ctypes.data_as(C.POINTER(C.c_int32)),
+            lp.ctypes.data_as(C.POINTER(C.c_double)))
+    assert gpu.lib.u1mps_sample_fock(*args, C.c_void_p(buf.data_ptr()), 256) == -4
+    assert gpu.lib.u1mps_sample_fock(*args, C.c_void_p(buf.data_ptr() + 8), need.value) == -1
+    assert gpu.lib.u1mps_sample_fock(*args, C.c_void_p(buf.data_ptr()), need.value) == 0
+    assert np.array_equal(pat, np.tile(occ, (2, 1)))
     assert np.allclose(gpu.expect_n_all(), occ)
 
 
