@@ -39,7 +39,7 @@ def test_static_scratch_matches_the_arena_path_on_two_calls_in_a_row():
     free_before = torch.cuda.mem_get_info()[0]
     gpu.expect_n_all_static(out2)
     torch.cuda.synchronize()
-    assert torch.cuda.mem_get_info()[0] == free_before          # nothing was allocated on the device
+    assert torch.cuda.mem_get_info()[0] >= free_before          # nothing was allocated on the device
     assert gpu.launch_count() == launches0 + 2                   # one kernel per call
     ref = gpu.expect_n_all()
     for out in (out1, out2):
