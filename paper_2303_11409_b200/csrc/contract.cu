@@ -3,9 +3,9 @@
 //                                         * Gamma^[s][c_l,c'] * lamC[c'] * Gamma^[s+1][c',c_r] ) * lamR[c_r]
 // One persistent grid walks the tile list built by the planner (variable-size sectors of all
 // gates of the chunk), 32 x 32 output tiles on FP64 tensor tiles (DMMA.8x8x4, 4 real MMAs per complex product).
-// The U entry is a scalar per K-chunk (the delta functions of Eq.16 "tell us
-// which entry of the unitary matrix to look up", L121), folded into the A operand together with
-// lambda^[k]; lambda^[k-1], lambda^[k+1] are applied in the epilogue.  The result is written straight
+// Minimum form: T(c') = Gamma^[s][c_l,c'] lamC[c'] Gamma^[s+1][c',c_r] is formed once per block pair (c_l, c_r) and
+// mixed into every Theta(c) with its U entry (the delta functions of Eq.16 "tell us which entry of the unitary matrix
+// to look up", L121); lambda^[k] is folded into the A operand, lambda^[k-1], lambda^[k+1] are applied in the epilogue.  The result is written straight
 // into the stacked column-major Jacobi matrix of the sector: Theta(c) if rows >= cols, else its
 // conjugate transpose, with the identity (accumulator of the right singular vectors) below it.
 #include "common.cuh"
@@ -28,7 +28,7 @@ __device__ __forceinline__ int upper_entry(const int* __restrict__ pref, int n, 
 }
 
 __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P, int G) {
-  __shared__ __align__(16) cplx As[KC * CT_LD];   // As[k][a]: (u lamC[k]) A[a0 + a][k0 + k]
+  __shared__ __align__(16) cplx As[KC * CT_LD];   // As[k][a]: lamC[k] A[a0 + a][k0 + k]
   __shared__ __align__(16) cplx Bs[KC * CT_LD];   // Bs[k][b]: B[k0 + k][b0 + b]
   const int NC = S.NC, d = S.d, dd = d * d, N = S.N;
   const int nf = G * NC * dd;
@@ -50,22 +50,32 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P
     const int tcols = u1_ceil_div(nR, U1_TILE);
     const int local = tile - P.t2pref[f];
     const int a0 = (local / tcols) * U1_TILE, b0 = (local % tcols) * U1_TILE;
-    const cplx* Ug = P.U + (long long)g * dd * dd + (long long)(i * d + j) * dd;  // row (out_s = i, out_{s+1} = j)
+    const cplx* Ug = P.U + (long long)g * dd * dd;
     const cplx* gA = S.gam + (long long)s * S.gcap;
     const cplx* gB = S.gam + (long long)(s + 1) * S.gcap;
-    double cre[4][2], cim[4][2];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) { cre[u][0] = cre[u][1] = 0.0; cim[u][0] = cim[u][1] = 0.0; }
+    // Minimum form of Eq.16: the block pair (c_l, c_r) occurs in Theta(c) for every c in [cplo, cphi], and the old centre
+    // charges c' run over the same range; T(c') = Gamma^[s][c_l,c'] lamC[c'] Gamma^[s+1][c',c_r] does not depend on c.
+    // The tile of the LOWEST c owns the pair: it forms each T(c') once and adds U[(c_l-c, c-c_r),(c_l-c', c'-c_r)] T(c')
+    // into the tile of every Theta(c) (first c' written, later ones read-modify-write by the same thread); the tiles of
+    // the other c have nothing to do.
     const int cplo = max(max(cr, cl - d + 1), 0), cphi = min(min(cl, cr + d - 1), N);
-    for (int cp = cplo; cp <= cphi; ++cp) {  // old centre sectors c' (the alpha_k sum of Eq.16, sector by sector)
-      const int nC = nbC[cp];
-      if (nC == 0) continue;
-      const cplx u = Ug[(cl - cp) * d + (cp - cr)];
+    if (c != cplo) continue;   // uniform over the CTA
+    const double* lamL = S.lam + (long long)s * S.chi + S.ob[(long long)s * NC + cl];
+    const double* lamR = S.lam + (long long)(s + 2) * S.chi + S.ob[(long long)(s + 2) * NC + cr];
+    bool first = true;
+    for (int cp = cplo; cp <= cphi + 1; ++cp) {  // old centre sectors c' (the alpha_k sum of Eq.16, sector by sector)
+      const bool flush = cp > cphi;              // after the last c': blocks that no c' reached are written as zeros
+      const int nC = flush ? 0 : nbC[cp];
+      if (flush ? !first : nC == 0) continue;
+      double cre[4][2], cim[4][2];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { cre[u][0] = cre[u][1] = 0.0; cim[u][0] = cim[u][1] = 0.0; }
+      if (!flush) {
       const cplx* A = gA + S.gamoff[((long long)s * NC + cl) * d + (cl - cp)];       // nL x nC
       const cplx* B = gB + S.gamoff[((long long)(s + 1) * NC + cp) * d + (cp - cr)];  // nC x nR
       const double* lamC = S.lam + (long long)(s + 1) * S.chi + S.ob[(long long)(s + 1) * NC + cp];
       for (int k0 = 0; k0 < nC; k0 += KC) {
-        // global -> registers (A: k fastest, B: b fastest: both coalesced), scale A by u lamC[k]
+        // global -> registers (A: k fastest, B: b fastest: both coalesced), scale A by lamC[k]
         cplx ra[4], rb[4];
         {
           const int k = tid & (KC - 1);
@@ -75,7 +85,8 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P
             cplx v = make_double2(0.0, 0.0);
             if (a0 + a < nL && k0 + k < nC) {
               const double l = lamC[k0 + k];
-              v = cmul(A[(long long)(a0 + a) * nC + k0 + k], make_double2(u.x * l, u.y * l));
+              v = A[(long long)(a0 + a) * nC + k0 + k];
+              v.x *= l; v.y *= l;
             }
             ra[x] = v;
           }
@@ -111,34 +122,41 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(DevState S, Plan P
           }
         }
       }
-    }
-    __syncthreads();  // before the next tile refills the stages
-    // epilogue: lambda^[k-1] on rows, lambda^[k+1] on columns, write into the stacked Jacobi matrix
-    int rowoff = 0, coloff = 0;
-    for (int ii = 0; ii < i; ++ii) rowoff += nbL[c + ii];
-    for (int jj = d - 1; jj > j; --jj) if (c - jj >= 0) coloff += nbR[c - jj];  // column blocks ascending c_r
-    const double* lamL = S.lam + (long long)s * S.chi + S.ob[(long long)s * NC + cl];
-    const double* lamR = S.lam + (long long)(s + 2) * S.chi + S.ob[(long long)(s + 2) * NC + cr];
-    const int rows = P.rows[e], cols = P.cols[e];
-    const bool tr = rows < cols;
-    const int ld = rows + cols;  // m + n
-    cplx* Wd = P.W + P.goff[e];
-    const int a = a0 + 8 * warp + lr;
-    if (a < nL) {
-      const double la = lamL[a];
+      __syncthreads();  // before the next c' (or the next tile) refills the stages
+      }   // (!flush)
+      // mix T(c') into every Theta(cc): lambda^[k-1] on rows, lambda^[k+1] on columns, into the stacked Jacobi matrices
+      for (int cc = cplo; cc <= cphi; ++cc) {
+        const int ec = g * NC + cc, ic = cl - cc, jc = cc - cr;
+        const cplx uu = flush ? make_double2(0.0, 0.0) : Ug[(long long)(ic * d + jc) * dd + (cl - cp) * d + (cp - cr)];
+        int rowoff = 0, coloff = 0;
+        for (int ii = 0; ii < ic; ++ii) rowoff += nbL[cc + ii];
+        for (int jj = d - 1; jj > jc; --jj) if (cc - jj >= 0) coloff += nbR[cc - jj];  // column blocks ascending c_r
+        const int rows = P.rows[ec], cols = P.cols[ec];
+        const bool tr = rows < cols;
+        const int ld = rows + cols;  // m + n
+        cplx* Wd = P.W + P.goff[ec];
+        const int a = a0 + 8 * warp + lr;
+        if (a < nL) {
+          const double la = lamL[a];
 #pragma unroll
-      for (int t = 0; t < 4; ++t)
+          for (int t = 0; t < 4; ++t)
 #pragma unroll
-        for (int x = 0; x < 2; ++x) {
-          const int b = b0 + 8 * t + 2 * lk + x;
-          if (b < nR) {
-            const double sc = la * lamR[b];
-            const cplx v = make_double2(cre[t][x] * sc, cim[t][x] * sc);
-            const long long r = rowoff + a, q = coloff + b;
-            if (!tr) Wd[r + q * ld] = v;
-            else Wd[q + r * ld] = make_double2(v.x, -v.y);
-          }
+            for (int x = 0; x < 2; ++x) {
+              const int b = b0 + 8 * t + 2 * lk + x;
+              if (b < nR) {
+                const double sc = la * lamR[b];
+                const double tr_ = cre[t][x] * sc, ti_ = cim[t][x] * sc;
+                cplx v = make_double2(uu.x * tr_ - uu.y * ti_, uu.x * ti_ + uu.y * tr_);
+                const long long r = rowoff + a, q = coloff + b;
+                cplx* dst = !tr ? &Wd[r + q * ld] : &Wd[q + r * ld];
+                if (tr) v.y = -v.y;
+                if (!first) { const cplx o = *dst; v.x += o.x; v.y += o.y; }
+                *dst = v;
+              }
+            }
         }
+      }
+      first = false;
     }
    }
   }
